@@ -1,0 +1,161 @@
+/*
+ * uniboost.h -- C-ABI of libuniboost.so: the per-iteration scheduling step of a
+ * continuous-batching LLM replica under the tail-aware scheduler of
+ * arxiv 2606.18431 (UniBoost), batched over R independent replicas and run as
+ * a trace-driven simulation on one B200 (sm_100a).
+ *
+ * Every step of the path runs in hand-written CUDA kernels; there is no CPU
+ * fallback.  Operation definitions (rules M1..M12) follow
+ *   Algorithm 1, PAPER.md:406-473   (rescore all active -> unified order ->
+ *                                    admit under KV capacity -> evict -> execute -> stats)
+ *   BOOST / QUANTIZE / SIGNAL,      PAPER.md:564-587, Eq. 2, Eq. 8
+ *   unified priority + hysteresis,  PAPER.md:185-196 (Eq. 7)
+ *   MemGuard minimum-run rule,
+ *   problem statement,              PAPER.md:117-123 (requests a_i, s_pre, s_dec), PAPER.md:409 (B, M, c, k, gamma)
+ * and the per-iteration cost model of BASELINE.json configs 1 and 3.
+ *
+ * Conventions
+ *  - every call returns UB_OK (0) or a negative UB_E* code; nothing throws or aborts across the ABI;
+ *  - "host" / "device" is stated per pointer; input arrays are caller-owned and copied (free after return);
+ *    outputs go to caller-allocated buffers; the handle owns all its device memory;
+ *  - the handle is not thread-safe; work is ordered on the borrowed CUDA stream; only the calls marked
+ *    "synchronises" wait for the device;
+ *  - all times are int64 microseconds; the only floating point is the host-side build of the boost table
+ *    (fp64, M4) and the final us -> s conversion of the statistics.
+ */
+#ifndef UNIBOOST_H
+#define UNIBOOST_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define UB_ABI_VERSION 1u
+#define UB_MAX_QUEUE   2048u      /* largest queue_cap (active requests per replica) */
+#define UB_TBT_BINS    4352u      /* log-linear TBT histogram, 7 sub-bits, gaps < 2^40 us (M11) */
+
+enum { UB_OK = 0, UB_EINVAL = -1, UB_ENOMEM = -2, UB_ECUDA = -3, UB_ESTATE = -4,
+       UB_EUNSORTED = -5, UB_EINFEASIBLE = -6, UB_ELIVELOCK = -7 };
+
+/* policy (M5): key = a | D-d | a - b_gamma(w_hat) | sig */
+enum { UB_FCFS = 0, UB_SRPT = 1, UB_BOOST = 2, UB_LAS = 3 };
+/* size signal (M3): P+d | SIGNAL of PAPER.md:575-587 | D-d (tests: SRPT limit) */
+enum { UB_SIG_UNIFIED = 0, UB_SIG_PHASE = 1, UB_SIG_REMAINING = 2 };
+/* quantiser (M3): Eq. 8 geometric bins | identity (vanilla boost, tests) */
+enum { UB_Q_GEOMETRIC = 0, UB_Q_EXACT = 1 };
+/* preemption (M8) */
+enum { UB_PRE_RECOMPUTE = 0, UB_PRE_SWAP = 1, UB_PRE_AUTO = 2 };
+
+typedef struct ub_sim ub_sim;     /* opaque */
+
+/* Simulator-wide parameters ("Require: B, M, c, k"; cost model BASELINE.json). */
+typedef struct {
+  uint32_t struct_size;           /* sizeof(ub_config), checked */
+  uint32_t abi_version;           /* UB_ABI_VERSION */
+  uint32_t n_replicas;            /* R >= 1 */
+  uint32_t n_traces;              /* distinct traces; replicas may share one */
+  uint32_t max_requests;          /* N: row length of the trace arrays */
+  uint32_t queue_cap;             /* Q: max simultaneously active requests per replica, 1..UB_MAX_QUEUE */
+  uint32_t kv_blocks;             /* B: KV capacity in blocks */
+  uint32_t block_tokens;          /* blk: tokens per block (16) */
+  uint32_t max_batch;             /* M: batch cap */
+  uint32_t chunk_tokens;          /* c: prefill chunk, 1..65535 */
+  uint32_t token_budget;          /* T: tokens per iteration, 1..65535 */
+  uint32_t preempt_mode;          /* UB_PRE_* */
+  uint32_t swap_ns_per_block;     /* swap time per block, ns (128 KiB / 25 GB/s = 5243) */
+  uint32_t swap_pool_blocks;      /* host swap pool, blocks */
+  uint32_t bin_tokens;            /* MemGuard k (Eq. 8) */
+  uint32_t tok_us;                /* service us credited per token in the argument of b_gamma (reading G1) */
+  int64_t  c0_us;                 /* iteration cost = c0 + c_prefill_tok * prefill tokens            */
+  int64_t  c_prefill_tok_us;      /*                + c_decode_seq * decode sequences + swap time (M9) */
+  int64_t  c_decode_seq_us;
+  uint32_t iters_per_launch;      /* scheduler iterations one kernel launch advances; 0 or 1 = one iteration per
+                                     launch with the state streamed HBM -> SM -> HBM every iteration */
+  int32_t  device;                /* CUDA device ordinal */
+  void*    stream;                /* cudaStream_t, borrowed; NULL = the legacy default stream */
+} ub_config;
+
+/* One per replica: policies / gamma points / trace seeds run side by side as the batch dimension. */
+typedef struct {
+  uint32_t trace_id;
+  uint8_t  policy;                /* UB_FCFS .. UB_LAS */
+  uint8_t  guard;                 /* MemGuard lock on/off */
+  uint8_t  signal_mode;           /* UB_SIG_* */
+  uint8_t  quant_mode;            /* UB_Q_* */
+  int64_t  hysteresis_us;         /* delta_hyst of Eq. 7, 0 .. 2^60 */
+  double   gamma;                 /* 1/s, > 0; +inf => boost 0 (== FCFS) */
+} ub_replica;
+
+/* Per-replica statistics (M11); identical field meaning to the oracle's. */
+typedef struct {
+  int64_t iterations, request_steps, n_completed;
+  int64_t evict_recompute, evict_swap, swapins;
+  int64_t tokens_lost, tokens_emitted, prefill_tokens, decode_seqs;
+  int64_t t_end_us, peak_active, done, swap_used;
+  int64_t ttft_us[3], ttlt_us[3], tbt_us[3];        /* P50, P90, P99: nearest rank */
+  int64_t sum_ttft_us, sum_ttlt_us, sum_tbt_num_us, sum_tbt_den;
+  double  ttft_s[3], ttlt_s[3], tbt_s[3];           /* the same in fp64 seconds */
+  double  mean_ttft_s, mean_ttlt_s, mean_tbt_s, tokens_per_s;
+} ub_replica_stats;
+
+/* Create a simulator.  cfg: host.  Allocates all device state for R replicas. */
+int  ub_create(const ub_config* cfg, ub_sim** out);
+void ub_destroy(ub_sim*);
+
+/* Load the request traces: [n_traces][max_requests] row-major, arrival-sorted per row,
+ * n_req[n_traces] valid requests per row.  Pointers are host (ptrs_on_device = 0) or device (1); the data
+ * is copied.  Validates on the device: UB_EUNSORTED if arrivals decrease, UB_EINFEASIBLE if some request has
+ * P < 1, D < 1 or ceil((P+D)/blk) > B, UB_EINVAL if an arrival is outside [0, 2^61].  Synchronises. */
+int  ub_load_trace(ub_sim*, const int64_t* arrival_us, const int32_t* prompt_tok, const int32_t* decode_tok,
+                   const uint32_t* n_req, int ptrs_on_device);
+
+/* Set the replica table (host, [R]) and reset every replica to t = 0 with an empty queue.  Builds the
+ * fixed-point boost table LUT[bin] = min(2^60, floor(b_gamma(k 2^bin tok_us 1e-6) 1e6 + 0.5)) us on the host
+ * in fp64 (Eq. 2, rule M4) and uploads it.  Needs a loaded trace.  Synchronises. */
+int  ub_set_replicas(ub_sim*, const ub_replica* reps);
+
+/* Advance every replica by n_iters scheduler iterations (a0..a5 of DESIGN.md Sec. 2: ingest, score, order,
+ * admit, victim-select, advance); finished replicas are no-ops.  Asynchronous on the stream unless
+ * live_replicas (host, nullable) is given: then it synchronises and returns the number of unfinished replicas. */
+int  ub_step(ub_sim*, uint32_t n_iters, uint64_t* live_replicas);
+
+/* Step until every replica is done or max_iters iterations were issued (then UB_ELIVELOCK).
+ * iters_done (host, nullable) = iterations issued.  Synchronises. */
+int  ub_run(ub_sim*, uint64_t max_iters, uint64_t* iters_done);
+
+/* Device-resident reduction of the per-request histories to P50/P90/P99 TTFT / TTLT / TBT, means and
+ * counters; out: host, [R].  Synchronises. */
+int  ub_stats(ub_sim*, ub_replica_stats* out);
+
+/* Per-request results, each [R][max_requests] (nullable): first / last token time (us, -1 = none yet),
+ * evictions, unforced evictions (victim was not MemGuard-locked).  Host (on_device = 0) or device.  Synchronises. */
+int  ub_per_request(ub_sim*, int64_t* t_first_us, int64_t* t_last_us, uint32_t* n_evict,
+                    uint32_t* n_evict_unforced, int on_device);
+
+/* Schedule digest H per replica (M12), host [R].  Equal digests + equal per-request results = identical
+ * schedule.  Synchronises. */
+int  ub_digest(ub_sim*, uint64_t* digest);
+
+/* Boost table of one replica: nb entries; lut (host, nullable) receives min(nb, cap).  */
+int  ub_boost_lut(ub_sim*, uint32_t replica, int64_t* lut, uint32_t cap, uint32_t* nb);
+
+/* TBT histogram of one replica, host [UB_TBT_BINS].  Synchronises. */
+int  ub_tbt_hist(ub_sim*, uint32_t replica, uint32_t* hist);
+
+/* Kernel-level parity: the active window of one replica in stored (= last priority) order.
+ * Each array host, [queue_cap], nullable; *n_active receives the count.  Synchronises. */
+int  ub_debug_get_state(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t* id, uint32_t* d,
+                        uint32_t* cached, uint32_t* flags, int64_t* clock_us);
+
+/* Timing of the step kernel launches issued by the LAST ub_step / ub_run call, measured with CUDA events on
+ * the borrowed stream: total milliseconds and launch count.  Synchronises. */
+int  ub_last_step_timing(ub_sim*, float* kernel_ms, uint32_t* launches);
+
+const char* ub_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

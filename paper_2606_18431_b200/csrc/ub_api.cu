@@ -1,0 +1,471 @@
+// ub_api.cu -- the C-ABI of libuniboost.so (include/uniboost.h): argument checking, device memory,
+// the host-side fp64 build of the fixed-point boost table (Eq. 2, rule M4) and the launch loops.
+// Every step of the scheduling path itself runs in the kernels of ub_step.cu / ub_aux.cu.
+#include "../../include/uniboost.h"
+#include "ub_internal.cuh"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <map>
+#include <new>
+#include <tuple>
+#include <vector>
+
+using namespace ub;
+
+struct ub_sim {
+  ub_config cfg;
+  SimDev dev;
+  cudaStream_t stream;
+  bool have_trace, have_reps;
+  // owned device memory
+  Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; RepPar* d_par; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
+  int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
+  StatsDev* d_stats; unsigned long long* d_word;
+  unsigned long long* h_word;            // pinned
+  std::vector<uint32_t> h_nreq, h_maxsig;
+  std::vector<ub_replica> h_reps;
+  std::vector<int64_t> h_lut;            // all tables back to back
+  std::vector<uint32_t> h_lut_off, h_lut_nb;
+  cudaEvent_t ev0, ev1;
+  float last_ms; uint32_t last_launches;
+};
+
+#define CK(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; } } while (0)
+
+static int set_dev(const ub_sim* s) { return cudaSetDevice(s->cfg.device) == cudaSuccess ? UB_OK : UB_ECUDA; }
+
+const char* ub_strerror(int e) {
+  switch (e) {
+    case UB_OK: return "ok";
+    case UB_EINVAL: return "invalid argument";
+    case UB_ENOMEM: return "out of memory";
+    case UB_ECUDA: return "CUDA error";
+    case UB_ESTATE: return "wrong call order";
+    case UB_EUNSORTED: return "arrivals not non-decreasing";
+    case UB_EINFEASIBLE: return "request does not fit the KV capacity or has P<1 or D<1";
+    case UB_ELIVELOCK: return "max_iters reached before all replicas finished";
+    default: return "unknown";
+  }
+}
+
+template <class T> static int dmalloc(T** p, size_t count) {
+  *p = nullptr;
+  cudaError_t e = cudaMalloc((void**)p, count ? count * sizeof(T) : sizeof(T));
+  if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return UB_ENOMEM; }
+  return e == cudaSuccess ? UB_OK : UB_ECUDA;
+}
+
+int ub_create(const ub_config* c, ub_sim** out) {
+  if (!c || !out) return UB_EINVAL;
+  *out = nullptr;
+  if (c->struct_size != sizeof(ub_config) || c->abi_version != UB_ABI_VERSION) return UB_EINVAL;
+  if (c->n_replicas < 1 || c->n_traces < 1 || c->max_requests < 1 || c->queue_cap < 1 ||
+      c->queue_cap > UB_MAX_QUEUE || c->kv_blocks < 1 || c->block_tokens < 1 || c->max_batch < 1 ||
+      c->chunk_tokens < 1 || c->chunk_tokens > 65535 || c->token_budget < 1 || c->token_budget > 65535 ||
+      c->c0_us < 0 || c->c_prefill_tok_us < 0 || c->c_decode_seq_us < 0 || c->preempt_mode > 2 ||
+      c->bin_tokens < 1 || c->tok_us < 1 || c->device < 0)
+    return UB_EINVAL;
+  // value ranges that keep every device quantity inside u32 / the flags word
+  if ((uint64_t)c->kv_blocks * c->block_tokens >= (1ull << 27) || c->bin_tokens >= (1u << 27) ||
+      c->c0_us > (1ll << 40) || c->c_prefill_tok_us > (1ll << 30) || c->c_decode_seq_us > (1ll << 30))
+    return UB_EINVAL;
+  if (cudaSetDevice(c->device) != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  ub_sim* s = new (std::nothrow) ub_sim();
+  if (!s) return UB_ENOMEM;
+  s->cfg = *c;
+  s->stream = (cudaStream_t)c->stream;
+  s->have_trace = s->have_reps = false;
+  s->d_TR = nullptr; s->d_lut = nullptr;
+  s->last_ms = 0.f; s->last_launches = 0;
+  const size_t R = c->n_replicas, Q = c->queue_cap, N = c->max_requests, NT = c->n_traces;
+  int rc = UB_OK;
+  if ((rc = dmalloc(&s->d_E0, R * Q)) || (rc = dmalloc(&s->d_E1, R * Q)) || (rc = dmalloc(&s->d_hdr, R)) ||
+      (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
+      (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
+      (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
+      (rc = dmalloc(&s->d_word, 2))) {
+    ub_destroy(s);
+    return rc;
+  }
+  if (cudaMallocHost((void**)&s->h_word, 2 * sizeof(unsigned long long)) != cudaSuccess ||
+      cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess ||
+      step_configure(c->queue_cap) != 0) {
+    cudaGetLastError();
+    ub_destroy(s);
+    return UB_ECUDA;
+  }
+  SimDev& d = s->dev;
+  memset(&d, 0, sizeof(d));
+  d.R = c->n_replicas; d.NT = c->n_traces; d.N = c->max_requests; d.Q = c->queue_cap;
+  d.B = c->kv_blocks; d.blk = c->block_tokens; d.M = c->max_batch; d.c = c->chunk_tokens; d.T = c->token_budget;
+  d.preempt_mode = c->preempt_mode; d.swap_ns = c->swap_ns_per_block; d.swap_pool = c->swap_pool_blocks;
+  d.k = c->bin_tokens; d.c0 = c->c0_us; d.c_pf = c->c_prefill_tok_us; d.c_dec = c->c_decode_seq_us;
+  d.E0 = s->d_E0; d.E1 = s->d_E1; d.hdr = s->d_hdr; d.par = s->d_par; d.n_req = s->d_nreq;
+  d.t_first = s->d_tfirst; d.t_last = s->d_tlast; d.n_evict = s->d_ne; d.n_evict_unf = s->d_neu; d.hist = s->d_hist;
+  *out = s;
+  return UB_OK;
+}
+
+void ub_destroy(ub_sim* s) {
+  if (!s) return;
+  cudaSetDevice(s->cfg.device);
+  cudaStreamSynchronize(s->stream);
+  cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_par); cudaFree(s->d_TR);
+  cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
+  cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
+  if (s->h_word) cudaFreeHost(s->h_word);
+  if (s->ev0) cudaEventDestroy(s->ev0);
+  if (s->ev1) cudaEventDestroy(s->ev1);
+  cudaGetLastError();
+  delete s;
+}
+
+int ub_load_trace(ub_sim* s, const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
+                  int on_device) {
+  if (!s || !a || !p || !d || !n_req) return UB_EINVAL;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t NT = s->cfg.n_traces, N = s->cfg.max_requests, tot = NT * N;
+  s->h_nreq.resize(NT);
+  if (on_device) CK(cudaMemcpy(s->h_nreq.data(), n_req, NT * 4, cudaMemcpyDeviceToHost));
+  else memcpy(s->h_nreq.data(), n_req, NT * 4);
+  for (size_t t = 0; t < NT; t++) if (s->h_nreq[t] > N) return UB_EINVAL;
+  s->have_trace = false; s->have_reps = false;
+  if (!s->d_TR) { int rc = dmalloc(&s->d_TR, tot); if (rc) return rc; }
+  CK(cudaMemcpyAsync(s->d_nreq, s->h_nreq.data(), NT * 4, cudaMemcpyHostToDevice, s->stream));
+  int64_t* da = nullptr; int32_t* dp = nullptr; int32_t* dd = nullptr;
+  const int64_t* ua = a; const int32_t* up = p; const int32_t* ud = d;
+  int rc = UB_OK;
+  if (!on_device) {
+    if ((rc = dmalloc(&da, tot)) || (rc = dmalloc(&dp, tot)) || (rc = dmalloc(&dd, tot))) {
+      cudaFree(da); cudaFree(dp); cudaFree(dd); return rc;
+    }
+    if (cudaMemcpyAsync(da, a, tot * 8, cudaMemcpyHostToDevice, s->stream) != cudaSuccess ||
+        cudaMemcpyAsync(dp, p, tot * 4, cudaMemcpyHostToDevice, s->stream) != cudaSuccess ||
+        cudaMemcpyAsync(dd, d, tot * 4, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) {
+      cudaGetLastError(); cudaFree(da); cudaFree(dp); cudaFree(dd); return UB_ECUDA;
+    }
+    ua = da; up = dp; ud = dd;
+  }
+  s->h_word[0] = ~0ull;
+  cudaMemcpyAsync(s->d_word, s->h_word, 8, cudaMemcpyHostToDevice, s->stream);
+  launch_pack_validate(ua, up, ud, s->d_nreq, (uint32_t)NT, (uint32_t)N, s->cfg.kv_blocks, s->cfg.block_tokens,
+                       s->d_TR, reinterpret_cast<int*>(s->d_word), s->stream);
+  cudaMemcpyAsync(s->h_word, s->d_word, 8, cudaMemcpyDeviceToHost, s->stream);
+  cudaError_t e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(da); cudaFree(dp); cudaFree(dd);
+  if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  if (s->h_word[0] != ~0ull) {
+    const int kind = (int)(s->h_word[0] & 3ull);
+    return kind == 0 ? UB_EINVAL : (kind == 1 ? UB_EUNSORTED : UB_EINFEASIBLE);
+  }
+  s->dev.TR = s->d_TR;
+  s->have_trace = true;
+  return UB_OK;
+}
+
+// Eq. 2 / BOOST in fixed point, rule M4:
+//   x = w_hat * tok_us * 1e-6 s;  b = (1/gamma) log(1/(1 - e^{-gamma x})) = -log(-expm1(-gamma x)) / gamma;
+//   table value = min(2^60, floor(b * 1e6 + 0.5)) us;  x == 0 -> 2^60;  gamma == +inf -> 0.
+static int64_t boost_table_entry(double gamma, double w_hat, uint32_t tok_us) {
+  if (isinf(gamma) && gamma > 0) return 0;
+  const double x = w_hat * (double)tok_us * 1e-6;
+  if (!(x > 0.0)) return kBoostMax;
+  const double b = -log(-expm1(-gamma * x)) / gamma;
+  const double v = floor(b * 1e6 + 0.5);
+  if (!(v > 0.0)) return 0;
+  if (v >= (double)kBoostMax) return kBoostMax;
+  return (int64_t)v;
+}
+
+// max over a trace of P + D (size of the EXACT-quantiser table), computed on the device copy
+__global__ void k_max_sig(const Rec0* TR, const uint32_t* n_req, uint32_t NT, uint32_t N, uint32_t* out) {
+  const uint32_t tr = blockIdx.x;
+  uint32_t m = 0;
+  for (uint32_t i = threadIdx.x; i < n_req[tr]; i += blockDim.x) {
+    const Rec0 q = TR[(size_t)tr * N + i];
+    m = max(m, q.P + q.D);
+  }
+  m = __reduce_max_sync(0xffffffffu, m);
+  if ((threadIdx.x & 31) == 0) atomicMax(out + tr, m);
+}
+
+int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
+  if (!s || !reps) return UB_EINVAL;
+  if (!s->have_trace) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const ub_config& c = s->cfg;
+  const size_t R = c.n_replicas, N = c.max_requests;
+  bool any_exact = false;
+  for (size_t r = 0; r < R; r++) {
+    const ub_replica& q = reps[r];
+    if (q.trace_id >= c.n_traces || q.policy > 3 || q.signal_mode > 2 || q.quant_mode > 1 || q.guard > 1 ||
+        q.hysteresis_us < 0 || q.hysteresis_us > (1ll << 60))
+      return UB_EINVAL;
+    if (q.policy == UB_BOOST && !(q.gamma > 0.0)) return UB_EINVAL;     // also rejects NaN
+    any_exact |= (q.quant_mode == UB_Q_EXACT);
+  }
+  s->have_reps = false;
+  if (any_exact) {
+    uint32_t* d_ms = nullptr;
+    int rc = dmalloc(&d_ms, c.n_traces); if (rc) return rc;
+    cudaMemsetAsync(d_ms, 0, c.n_traces * 4, s->stream);
+    k_max_sig<<<c.n_traces, 128, 0, s->stream>>>(s->d_TR, s->d_nreq, c.n_traces, c.max_requests, d_ms);
+    s->h_maxsig.resize(c.n_traces);
+    cudaError_t e = cudaMemcpyAsync(s->h_maxsig.data(), d_ms, c.n_traces * 4, cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    cudaFree(d_ms);
+    if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  }
+  // boost tables, one per distinct (gamma, quantiser, length); non-BOOST policies never read one
+  s->h_reps.assign(reps, reps + R);
+  s->h_lut.clear(); s->h_lut_off.assign(R, 0); s->h_lut_nb.assign(R, 0);
+  std::map<std::tuple<uint64_t, uint32_t, uint32_t>, uint32_t> seen;
+  std::vector<RepPar> par(R);
+  for (size_t r = 0; r < R; r++) {
+    const ub_replica& q = reps[r];
+    const uint32_t nb = (q.quant_mode == UB_Q_EXACT) ? s->h_maxsig[q.trace_id] + 1u : 64u;
+    uint32_t off = 0;
+    if (q.policy == UB_BOOST) {
+      uint64_t gb; memcpy(&gb, &q.gamma, 8);
+      auto key = std::make_tuple(gb, (uint32_t)q.quant_mode, nb);
+      auto it = seen.find(key);
+      if (it != seen.end()) off = it->second;
+      else {
+        if (s->h_lut.size() + nb >= (1ull << 32)) return UB_ENOMEM;
+        off = (uint32_t)s->h_lut.size();
+        seen.emplace(key, off);
+        for (uint32_t b = 0; b < nb; b++) {
+          const double w_hat = (q.quant_mode == UB_Q_EXACT) ? (double)b : ldexp((double)c.bin_tokens, (int)b);
+          s->h_lut.push_back(boost_table_entry(q.gamma, w_hat, c.tok_us));
+        }
+      }
+    }
+    s->h_lut_off[r] = off; s->h_lut_nb[r] = nb;
+    RepPar& p = par[r];
+    p.delta = q.hysteresis_us; p.trace_id = q.trace_id; p.lut_off = off; p.lut_nb = nb;
+    p.policy = q.policy; p.guard = q.guard; p.signal_mode = q.signal_mode; p.quant_mode = q.quant_mode;
+  }
+  cudaFree(s->d_lut); s->d_lut = nullptr;
+  int rc = dmalloc(&s->d_lut, s->h_lut.size()); if (rc) return rc;
+  if (!s->h_lut.empty())
+    CK(cudaMemcpyAsync(s->d_lut, s->h_lut.data(), s->h_lut.size() * 8, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->d_par, par.data(), R * sizeof(RepPar), cudaMemcpyHostToDevice, s->stream));
+  s->dev.lut = s->d_lut;
+  // reset the run state
+  CK(cudaMemsetAsync(s->d_tfirst, 0xFF, R * N * 8, s->stream));     // -1
+  CK(cudaMemsetAsync(s->d_tlast, 0xFF, R * N * 8, s->stream));
+  CK(cudaMemsetAsync(s->d_ne, 0, R * N * 4, s->stream));
+  CK(cudaMemsetAsync(s->d_neu, 0, R * N * 4, s->stream));
+  CK(cudaMemsetAsync(s->d_hist, 0, R * (size_t)kTbtBins * 4, s->stream));
+  launch_reset(s->dev, s->stream);
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaGetLastError());
+  s->have_reps = true;
+  return UB_OK;
+}
+
+static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
+  const uint32_t ipl = s->cfg.iters_per_launch > 1 ? s->cfg.iters_per_launch : 1;
+  uint32_t nl = 0;
+  while (n_iters > 0) {
+    const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
+    launch_step(s->dev, k, s->stream);
+    n_iters -= k; nl++;
+  }
+  *launches = nl;
+  return cudaGetLastError() == cudaSuccess ? UB_OK : UB_ECUDA;
+}
+
+static int read_live(ub_sim* s, uint64_t* live) {
+  launch_count_live(s->dev, s->d_word, s->stream);
+  CK(cudaMemcpyAsync(s->h_word, s->d_word, 8, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaGetLastError());
+  *live = s->h_word[0];
+  return UB_OK;
+}
+
+int ub_step(ub_sim* s, uint32_t n_iters, uint64_t* live) {
+  if (!s) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  CK(cudaEventRecord(s->ev0, s->stream));
+  uint32_t nl = 0;
+  int rc = issue_steps(s, n_iters, &nl);
+  CK(cudaEventRecord(s->ev1, s->stream));
+  s->last_launches = nl; s->last_ms = -1.f;
+  if (rc) return rc;
+  if (live) return read_live(s, live);
+  return UB_OK;
+}
+
+int ub_run(ub_sim* s, uint64_t max_iters, uint64_t* iters_done) {
+  if (!s) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  uint64_t done = 0, live = 1;
+  uint32_t total_launches = 0;
+  float total_ms = 0.f;
+  int rc = read_live(s, &live);
+  if (rc) return rc;
+  uint64_t chunk = 256;
+  while (live > 0 && done < max_iters) {
+    const uint64_t k = (max_iters - done) < chunk ? (max_iters - done) : chunk;
+    uint32_t nl = 0;
+    CK(cudaEventRecord(s->ev0, s->stream));
+    rc = issue_steps(s, k, &nl);
+    CK(cudaEventRecord(s->ev1, s->stream));
+    if (rc) return rc;
+    done += k; total_launches += nl;
+    if ((rc = read_live(s, &live))) return rc;
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, s->ev0, s->ev1));
+    total_ms += ms;
+    if (chunk < 4096) chunk *= 2;
+  }
+  s->last_ms = total_ms; s->last_launches = total_launches;
+  if (iters_done) *iters_done = done;
+  return live > 0 ? UB_ELIVELOCK : UB_OK;
+}
+
+int ub_last_step_timing(ub_sim* s, float* ms, uint32_t* launches) {
+  if (!s) return UB_EINVAL;
+  if (set_dev(s)) return UB_ECUDA;
+  if (s->last_ms < 0.f) {
+    CK(cudaEventSynchronize(s->ev1));
+    float v = 0.f;
+    CK(cudaEventElapsedTime(&v, s->ev0, s->ev1));
+    s->last_ms = v;
+  }
+  if (ms) *ms = s->last_ms;
+  if (launches) *launches = s->last_launches;
+  return UB_OK;
+}
+
+int ub_stats(ub_sim* s, ub_replica_stats* out) {
+  if (!s || !out) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t R = s->cfg.n_replicas;
+  launch_stats(s->dev, s->d_stats, s->stream);
+  std::vector<StatsDev> sd(R);
+  std::vector<Hdr> hd(R);
+  CK(cudaMemcpyAsync(sd.data(), s->d_stats, R * sizeof(StatsDev), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaMemcpyAsync(hd.data(), s->d_hdr, R * sizeof(Hdr), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaGetLastError());
+  for (size_t r = 0; r < R; r++) {
+    const Hdr& h = hd[r];
+    ub_replica_stats& o = out[r];
+    memset(&o, 0, sizeof(o));
+    o.iterations = h.iterations; o.request_steps = h.request_steps; o.n_completed = h.n_completed;
+    o.evict_recompute = h.evict_recompute; o.evict_swap = h.evict_swap; o.swapins = h.swapins;
+    o.tokens_lost = h.tokens_lost; o.tokens_emitted = h.tokens_emitted;
+    o.prefill_tokens = h.prefill_tokens; o.decode_seqs = h.decode_seqs;
+    o.t_end_us = h.t; o.peak_active = h.peak_active; o.swap_used = h.swap_used;
+    o.done = (h.n_active == 0 && h.next >= s->h_nreq[s->h_reps[r].trace_id]) ? 1 : 0;
+    o.sum_ttft_us = h.sum_ttft; o.sum_ttlt_us = h.sum_ttlt;
+    o.sum_tbt_num_us = h.sum_tbt_num; o.sum_tbt_den = h.sum_tbt_den;
+    for (int k = 0; k < 3; k++) {
+      o.ttft_us[k] = sd[r].ttft[k]; o.ttlt_us[k] = sd[r].ttlt[k]; o.tbt_us[k] = sd[r].tbt[k];
+      o.ttft_s[k] = (double)o.ttft_us[k] * 1e-6;      // final us -> s in fp64 (M11)
+      o.ttlt_s[k] = (double)o.ttlt_us[k] * 1e-6;
+      o.tbt_s[k] = (double)o.tbt_us[k] * 1e-6;
+    }
+    const int64_t m = h.n_completed;
+    o.mean_ttft_s = m ? ((double)h.sum_ttft / (double)m) * 1e-6 : 0.0;
+    o.mean_ttlt_s = m ? ((double)h.sum_ttlt / (double)m) * 1e-6 : 0.0;
+    o.mean_tbt_s = h.sum_tbt_den ? ((double)h.sum_tbt_num / (double)h.sum_tbt_den) * 1e-6 : 0.0;
+    o.tokens_per_s = h.t > 0 ? (double)h.tokens_emitted / ((double)h.t * 1e-6) : 0.0;
+  }
+  return UB_OK;
+}
+
+__global__ void k_mask_done(const uint32_t* in, uint32_t* out, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    out[i] = in[i] & 0x7FFFFFFFu;
+}
+
+int ub_per_request(ub_sim* s, int64_t* tf, int64_t* tl, uint32_t* ne, uint32_t* neu, int on_device) {
+  if (!s) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t tot = (size_t)s->cfg.n_replicas * s->cfg.max_requests;
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  launch_flush_tlast(s->dev, s->stream);
+  if (tf) CK(cudaMemcpyAsync(tf, s->d_tfirst, tot * 8, kind, s->stream));
+  if (tl) CK(cudaMemcpyAsync(tl, s->d_tlast, tot * 8, kind, s->stream));
+  if (neu) CK(cudaMemcpyAsync(neu, s->d_neu, tot * 4, kind, s->stream));
+  if (ne) {
+    if (on_device) {
+      k_mask_done<<<148 * 8, 256, 0, s->stream>>>(s->d_ne, ne, tot);
+    } else {
+      CK(cudaMemcpyAsync(ne, s->d_ne, tot * 4, kind, s->stream));
+    }
+  }
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaGetLastError());
+  if (ne && !on_device) for (size_t i = 0; i < tot; i++) ne[i] &= 0x7FFFFFFFu;   // bit 31 is the completion marker
+  return UB_OK;
+}
+
+int ub_digest(ub_sim* s, uint64_t* dg) {
+  if (!s || !dg) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t R = s->cfg.n_replicas;
+  CK(cudaMemcpy2DAsync(dg, 8, reinterpret_cast<const char*>(s->d_hdr) + offsetof(Hdr, H), sizeof(Hdr), 8, R,
+                       cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return UB_OK;
+}
+
+int ub_boost_lut(ub_sim* s, uint32_t r, int64_t* lut, uint32_t cap, uint32_t* nb) {
+  if (!s || !nb || r >= s->cfg.n_replicas) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  const uint32_t n = s->h_lut_nb[r];
+  *nb = n;
+  if (lut) {
+    const bool boost = s->h_reps[r].policy == UB_BOOST;
+    for (uint32_t b = 0; b < n && b < cap; b++) lut[b] = boost ? s->h_lut[s->h_lut_off[r] + b] : 0;
+  }
+  return UB_OK;
+}
+
+int ub_tbt_hist(ub_sim* s, uint32_t r, uint32_t* hist) {
+  if (!s || !hist || r >= s->cfg.n_replicas) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  CK(cudaMemcpyAsync(hist, s->d_hist + (size_t)r * kTbtBins, kTbtBins * 4, cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  return UB_OK;
+}
+
+int ub_debug_get_state(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint32_t* d, uint32_t* cached,
+                       uint32_t* flags, int64_t* clock_us) {
+  if (!s || r >= s->cfg.n_replicas) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  Hdr h;
+  CK(cudaMemcpyAsync(&h, s->d_hdr + r, sizeof(Hdr), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  std::vector<Rec1> e(h.n_active);
+  if (h.n_active) {
+    CK(cudaMemcpyAsync(e.data(), s->d_E1 + (size_t)r * s->cfg.queue_cap, h.n_active * sizeof(Rec1),
+                       cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
+  if (n_active) *n_active = h.n_active;
+  if (clock_us) *clock_us = h.t;
+  for (uint32_t i = 0; i < h.n_active; i++) {
+    if (id) id[i] = e[i].id;
+    if (d) d[i] = e[i].d;
+    if (cached) cached[i] = e[i].cached;
+    if (flags) flags[i] = e[i].flags;
+  }
+  return UB_OK;
+}

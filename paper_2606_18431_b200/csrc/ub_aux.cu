@@ -1,0 +1,192 @@
+// ub_aux.cu -- the kernels around the scheduling step: trace validation + packing, reset, live count,
+// t_last flush, and the device-resident percentile reduction a6 (M11; t_p of PAPER.md:225).
+#include "ub_internal.cuh"
+
+namespace ub {
+
+// ------------------------------------------------------------------ trace validation + packing (ub_load_trace)
+// err: first offending (trace, request) in row-major scan order, encoded (linear index << 2 | kind),
+// kind 0 = arrival outside [0, 2^61] (UB_EINVAL), 1 = arrivals decrease (UB_EUNSORTED), 2 = infeasible request.
+__global__ void k_pack_validate(const int64_t* __restrict__ a, const int32_t* __restrict__ p,
+                                const int32_t* __restrict__ d, const uint32_t* __restrict__ n_req,
+                                uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* __restrict__ out,
+                                unsigned long long* err) {
+  const size_t total = (size_t)NT * N;
+  for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
+    const uint32_t tr = (uint32_t)(g / N), i = (uint32_t)(g % N);
+    Rec0 rec; rec.a = a[g]; rec.P = (uint32_t)p[g]; rec.D = (uint32_t)d[g];
+    out[g] = rec;
+    if (i >= n_req[tr]) continue;
+    const int64_t ai = rec.a;
+    const int64_t P = p[g], D = d[g];
+    int kind = -1;
+    if (ai < 0 || ai > ((int64_t)1 << 61)) kind = 0;
+    else if (i > 0 && ai < a[g - 1]) kind = 1;
+    else if (P < 1 || D < 1 || (P + D + blk - 1) / blk > (int64_t)B) kind = 2;
+    if (kind >= 0) atomicMin(err, ((unsigned long long)g << 2) | (unsigned long long)kind);
+  }
+}
+
+void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
+                          uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st) {
+  const size_t total = (size_t)NT * N;
+  int blocks = (int)((total + 255) / 256);
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  if (blocks < 1) blocks = 1;
+  k_pack_validate<<<blocks, 256, 0, st>>>(a, p, d, n_req, NT, N, B, blk, out,
+                                          reinterpret_cast<unsigned long long*>(err));
+}
+
+// ------------------------------------------------------------------ reset (ub_set_replicas)
+__global__ void k_reset(SimDev s) {
+  const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= s.R) return;
+  Hdr h;
+  memset(&h, 0, sizeof(h));
+  const uint32_t tr = s.par[r].trace_id;
+  h.a_next = (s.n_req[tr] > 0) ? s.TR[(size_t)tr * s.N].a : kNever;
+  s.hdr[r] = h;
+}
+void launch_reset(const SimDev& s, cudaStream_t st) { k_reset<<<(s.R + 127) / 128, 128, 0, st>>>(s); }
+
+// ------------------------------------------------------------------ live replicas (ub_step / ub_run)
+__global__ void k_count_live(SimDev s, unsigned long long* live) {
+  const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+  int alive = 0;
+  if (r < s.R) {
+    const Hdr* h = s.hdr + r;
+    alive = !(h->n_active == 0 && h->next >= s.n_req[s.par[r].trace_id]);
+  }
+  const int c = __syncthreads_count(alive);
+  if (threadIdx.x == 0 && c) atomicAdd(live, (unsigned long long)c);
+}
+void launch_count_live(const SimDev& s, unsigned long long* live, cudaStream_t st) {
+  cudaMemsetAsync(live, 0, sizeof(unsigned long long), st);
+  k_count_live<<<(s.R + 255) / 256, 256, 0, st>>>(s, live);
+}
+
+// ------------------------------------------------------------------ t_last flush (ub_per_request)
+// A request that emitted in the last executed iteration carries its t_last implicitly (== replica clock).
+__global__ void k_flush_tlast(SimDev s) {
+  const uint32_t r = blockIdx.x;
+  const Hdr* h = s.hdr + r;
+  const uint32_t n = h->n_active;
+  const int64_t t = h->t;
+  const Rec1* e1 = s.E1 + (size_t)r * s.Q;
+  for (uint32_t p = threadIdx.x; p < n; p += blockDim.x) {
+    const Rec1 r1 = e1[p];
+    if (r1.flags & F_EMITPREV) s.t_last[(size_t)r * s.N + r1.id] = t;
+  }
+}
+void launch_flush_tlast(const SimDev& s, cudaStream_t st) { k_flush_tlast<<<s.R, 128, 0, st>>>(s); }
+
+// ------------------------------------------------------------------ a6: percentile reduction (M11)
+// Nearest rank: the ceil(p m / 100)-th smallest of the m completed requests' TTFT_i = t_first - a_i and
+// TTLT_i = t_last - a_i, found exactly by an MSD radix select (8 passes of 8 bits) over values recomputed
+// on the fly from HBM (L2-resident after the first pass); TBT from the pooled log-linear histogram.
+constexpr int kStatThreads = 256;
+constexpr uint32_t kDoneBit = 0x80000000u;      // n_evict bit 31 marks a completed request
+
+__device__ __forceinline__ int64_t tbt_edge(uint32_t idx) {
+  int sft = (int)(idx / 128) - 1; if (sft < 0) sft = 0;
+  return (int64_t)(idx - 128u * (uint32_t)sft) << sft;
+}
+
+__global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out) {
+  __shared__ uint32_t hist[256];
+  __shared__ uint32_t wtot[kStatThreads / 32];
+  __shared__ unsigned long long sel_prefix;
+  __shared__ uint32_t sel_rank;
+  const uint32_t r = blockIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t tr = s.par[r].trace_id, nreq = s.n_req[tr];
+  const Rec0* TR = s.TR + (size_t)tr * s.N;
+  const int64_t* tf = s.t_first + (size_t)r * s.N;
+  const int64_t* tl = s.t_last + (size_t)r * s.N;
+  const uint32_t* ne = s.n_evict + (size_t)r * s.N;
+  const uint32_t m = s.hdr[r].n_completed;
+  const int pct[3] = {50, 90, 99};
+
+  for (int which = 0; which < 2; which++) {
+    const int64_t* src = which == 0 ? tf : tl;
+    for (int k = 0; k < 3; k++) {
+      int64_t result = 0;
+      if (m > 0) {
+        uint64_t rank = ((uint64_t)pct[k] * m + 99) / 100;
+        if (rank < 1) rank = 1;
+        if (rank > m) rank = m;
+        if (tid == 0) { sel_prefix = 0ull; sel_rank = (uint32_t)(rank - 1); }
+        for (int pass = 7; pass >= 0; pass--) {
+          hist[tid] = 0;
+          __syncthreads();
+          const unsigned long long prefix = sel_prefix;
+          const int sh_hi = 8 * (pass + 1);
+          for (uint32_t i = tid; i < nreq; i += kStatThreads) {
+            if (!(ne[i] & kDoneBit)) continue;
+            const unsigned long long v = (unsigned long long)(src[i] - TR[i].a);
+            const bool match = (pass == 7) || ((v >> sh_hi) == (prefix >> sh_hi));
+            if (match) atomicAdd(&hist[(v >> (8 * pass)) & 0xFF], 1u);
+          }
+          __syncthreads();
+          // bucket holding the sel_rank-th (0-based) matching value: thread b owns bucket b
+          const uint32_t cntb = hist[tid];
+          uint32_t inc = cntb;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += x; }
+          if (lane == 31) wtot[warp] = inc;
+          __syncthreads();
+          uint32_t off = 0;
+          for (int w = 0; w < warp; w++) off += wtot[w];
+          inc += off;
+          const uint32_t exc = inc - cntb, want = sel_rank;
+          __syncthreads();
+          if (want >= exc && want < inc) {
+            sel_prefix = prefix | ((unsigned long long)tid << (8 * pass));
+            sel_rank = want - exc;
+          }
+          __syncthreads();
+        }
+        result = (int64_t)sel_prefix;
+      }
+      if (tid == 0) { if (which == 0) out[r].ttft[k] = result; else out[r].ttlt[k] = result; }
+      __syncthreads();
+    }
+  }
+
+  // TBT: thread i owns bins [17 i, 17 i + 17)
+  {
+    const uint32_t* gh = s.hist + (size_t)r * kTbtBins;
+    constexpr int per = kTbtBins / kStatThreads;      // 17
+    uint32_t loc[per];
+    uint32_t sum = 0;
+#pragma unroll
+    for (int b = 0; b < per; b++) { loc[b] = gh[tid * per + b]; sum += loc[b]; }
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += x; }
+    if (lane == 31) wtot[warp] = inc;
+    __syncthreads();
+    uint64_t off = 0, total = 0;
+    for (int w = 0; w < kStatThreads / 32; w++) { if (w < warp) off += wtot[w]; total += wtot[w]; }
+    const uint64_t incl = off + inc, excl = incl - sum;
+    for (int k = 0; k < 3; k++) {
+      if (total == 0) { if (tid == 0) out[r].tbt[k] = 0; continue; }
+      uint64_t rank = ((uint64_t)pct[k] * total + 99) / 100;
+      if (rank < 1) rank = 1;
+      if (rank > excl && rank <= incl) {
+        uint64_t cum = excl;
+#pragma unroll
+        for (int b = 0; b < per; b++) {
+          cum += loc[b];
+          if (cum >= rank) { out[r].tbt[k] = tbt_edge((uint32_t)(tid * per + b)); break; }
+        }
+      }
+    }
+  }
+}
+
+void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st) { k_stats<<<s.R, kStatThreads, 0, st>>>(s, out); }
+size_t stats_smem_bytes(uint32_t) { return 0; }
+int stats_configure(uint32_t) { return 0; }
+
+}  // namespace ub

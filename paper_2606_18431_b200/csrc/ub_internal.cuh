@@ -1,0 +1,87 @@
+// ub_internal.cuh -- device-side data layout shared by the kernels and the C-ABI host code of libuniboost.so.
+// (Nothing here is shared with oracle/.)
+//
+// HBM layout.  Per replica r the active window is a struct of two 16-byte record
+// arrays kept in PRIORITY ORDER of the last executed iteration (so the next iteration finds it nearly sorted):
+//   E0[r][Q] = { a: i64 arrival us, P: u32 prompt tokens, D: u32 hidden output tokens }   static per request
+//   E1[r][Q] = { id: u32, d: u32 tokens emitted, cached: u32 KV tokens held, flags: u32 } dynamic
+// plus one 160-byte header Hdr[r], the packed traces TR[trace][N] (same 16-byte record as E0), the
+// per-request outputs t_first/t_last/n_evict/n_evict_unforced [R][N] and the TBT histogram [R][4352].
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace ub {
+
+constexpr int      kTbtBins   = 4352;
+constexpr uint32_t kMaxQueue  = 2048;
+constexpr int64_t  kBoostMax  = (int64_t)1 << 60;
+constexpr int64_t  kKeyBias   = (int64_t)1 << 62;
+constexpr int64_t  kNever     = INT64_MAX;          // a_next when the trace is exhausted
+
+// flags word of E1
+constexpr uint32_t F_RESIDENT = 1u;        // KV on the device
+constexpr uint32_t F_SWAPPED  = 2u;        // KV in the host swap pool
+constexpr uint32_t F_EMITPREV = 4u;        // emitted a token in the previous executed iteration => t_last == clock
+constexpr uint32_t F_DIRTY    = 8u;        // hint: (class,key) may differ from the previous iteration's
+constexpr int      F_LOCK_SHIFT = 4;       // bits 4..31: lockbin + 1 (0 = no lock)
+
+struct __align__(16) Rec0 { int64_t a; uint32_t P; uint32_t D; };
+struct __align__(16) Rec1 { uint32_t id; uint32_t d; uint32_t cached; uint32_t flags; };
+
+struct __align__(16) Hdr {
+  int64_t  t;                 // replica clock, us
+  uint64_t H;                 // schedule digest (M12)
+  int64_t  a_next;            // arrival of trace[next], kNever if exhausted
+  int64_t  request_steps;
+  int64_t  tokens_emitted, prefill_tokens, decode_seqs, tokens_lost;
+  int64_t  sum_ttft, sum_ttlt, sum_tbt_num, sum_tbt_den;
+  int64_t  iterations;
+  uint32_t n_active, next, swap_used, peak_active;
+  uint32_t n_completed, evict_recompute, evict_swap, swapins;
+  uint32_t done, pad0, pad1, pad2;
+};
+static_assert(sizeof(Hdr) == 160, "Hdr is 160 bytes");
+
+struct __align__(8) RepPar {    // per-replica parameters, read-only on the device
+  int64_t  delta;               // hysteresis_us
+  uint32_t trace_id;
+  uint32_t lut_off;             // offset of this replica's boost table in lut[]
+  uint32_t lut_nb;              // entries
+  uint8_t  policy, guard, signal_mode, quant_mode;
+};
+
+struct SimDev {                 // kernel argument (by value)
+  // configuration
+  uint32_t R, NT, N, Q;
+  uint32_t B, blk, M, c, T;
+  uint32_t preempt_mode, swap_ns, swap_pool, k;
+  int64_t  c0, c_pf, c_dec;
+  // state
+  Rec0* E0; Rec1* E1; Hdr* hdr;
+  const RepPar* par;
+  const Rec0* TR;               // packed traces [NT][N]
+  const uint32_t* n_req;        // [NT]
+  const int64_t* lut;
+  int64_t* t_first; int64_t* t_last;      // [R][N]
+  uint32_t* n_evict; uint32_t* n_evict_unf;
+  uint32_t* hist;               // [R][kTbtBins]
+};
+
+// kernels (ub_step.cu, ub_aux.cu)
+void launch_step(const SimDev& s, uint32_t iters, cudaStream_t st);
+size_t step_smem_bytes(uint32_t Q);
+int  step_configure(uint32_t Q);
+void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
+                          uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st);
+void launch_reset(const SimDev& s, cudaStream_t st);
+void launch_count_live(const SimDev& s, unsigned long long* live, cudaStream_t st);
+void launch_flush_tlast(const SimDev& s, cudaStream_t st);
+struct StatsDev {               // device-side result of the percentile reduction, one per replica
+  int64_t ttft[3], ttlt[3], tbt[3];
+};
+void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st);
+size_t stats_smem_bytes(uint32_t N);
+int  stats_configure(uint32_t N);
+
+}  // namespace ub

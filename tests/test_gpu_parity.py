@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path (through the C-ABI of libuniboost.so) against the CPU oracle, element by element,
+on the same seeded inputs.  Bar (north_star): the whole schedule bit-exact -- boost table, per-iteration digest,
+per-request (t_first, t_last, n_evict), counters, integer-microsecond percentiles -- and the fp64 percentiles in
+seconds within 1e-9 relative (they are the same integers times 1e-6, so in fact equal).
+"""
+import numpy as np
+import pytest
+
+from paper_2606_18431_b200 import workloads as W
+from tests.helpers import pressure_workload
+
+pytestmark = pytest.mark.gpu
+
+INT_STATS = ("iterations", "request_steps", "n_completed", "evict_recompute", "evict_swap", "swapins",
+             "tokens_lost", "tokens_emitted", "prefill_tokens", "decode_seqs", "t_end_us", "peak_active", "done",
+             "swap_used", "ttft_us", "ttlt_us", "tbt_us", "sum_ttft_us", "sum_ttlt_us", "sum_tbt_num_us",
+             "sum_tbt_den")
+F64_STATS = ("ttft_s", "ttlt_s", "tbt_s", "mean_ttft_s", "mean_ttlt_s", "mean_tbt_s", "tokens_per_s")
+REL_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    from paper_2606_18431_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _pair(gpu, oracle_mod, wl, ipl=1, workers=1):
+    tr = wl.traces(workers=workers)
+    g = gpu.Sim(wl.sim, wl.replicas, tr, iters_per_launch=ipl)
+    o = oracle_mod.OracleSim(wl.sim, wl.replicas, tr)
+    return g, o
+
+
+def _assert_same(g, o, where=""):
+    dg, do = g.digest(), o.digest()
+    bad = np.nonzero(dg != do)[0]
+    assert bad.size == 0, f"{where}: digest differs on replicas {bad[:8]} ({bad.size} of {len(dg)})"
+    gtf, gtl, gne, gneu = g.per_request()
+    otf, otl, one, oneu = o.per_request()
+    assert np.array_equal(gtf, otf), f"{where}: t_first"
+    assert np.array_equal(gtl, otl), f"{where}: t_last"
+    assert np.array_equal(gne, one), f"{where}: n_evict"
+    assert np.array_equal(gneu, oneu), f"{where}: n_evict_unforced"
+    gs, os_ = g.stats(), o.stats()
+    for r, (a, b) in enumerate(zip(gs, os_)):
+        for k in INT_STATS:
+            assert a[k] == b[k], f"{where}: replica {r} stat {k}: gpu {a[k]} oracle {b[k]}"
+        for k in F64_STATS:
+            av, bv = np.atleast_1d(a[k]).astype(float), np.atleast_1d(b[k]).astype(float)
+            assert np.all(np.abs(av - bv) <= REL_TOL * np.maximum(1e-300, np.abs(bv))), f"{where}: replica {r} {k}"
+
+
+def _assert_hist_same(g, o, reps):
+    for r in reps:
+        assert np.array_equal(g.tbt_hist(r), o.tbt_hist(r)), f"TBT histogram of replica {r}"
+
+
+# ------------------------------------------------------------------------------------------ boost table (M4)
+
+@pytest.mark.parametrize("gamma", [0.01, 0.05, 0.3, 1.0, 10.0, 100.0, float("inf"), 1e-7])
+@pytest.mark.parametrize("quant", [W.QUANT_GEOMETRIC, W.QUANT_EXACT])
+def test_boost_table_bit_exact(gpu, oracle_mod, gamma, quant):
+    wl = pressure_workload(1, n=40, gamma=gamma, quant=quant)
+    g, o = _pair(gpu, oracle_mod, wl)
+    assert np.array_equal(g.boost_lut(0), o.boost_lut(0))
+
+
+# ------------------------------------------------------------------------------------------ config 1 in full
+
+def test_config1_full_schedule(gpu, oracle_mod):
+    wl = W.config1()
+    g, o = _pair(gpu, oracle_mod, wl)
+    g.run(); o.run()
+    _assert_same(g, o, "config1")
+    _assert_hist_same(g, o, [0])
+    st = g.stats()[0]
+    assert st["done"] == 1 and st["n_completed"] == 256
+
+
+def test_config1_step_by_step(gpu, oracle_mod):
+    """Digest, clock and the active window (id, d, cached, resident) after every single iteration."""
+    wl = W.config1()
+    g, o = _pair(gpu, oracle_mod, wl)
+    for it in range(3000):
+        g.step(1)
+        info, rows = o.step_replica(0)
+        st = g.debug_state(0)
+        assert g.digest()[0] == o.digest()[0], f"iteration {it}"
+        assert st["clock_us"] == info["t_end_us"]
+        live = [(r["id"], r["d_after"], r["cached_after"], r["resident_after"]) for r in rows
+                if not (r["want"] > 0 and r["cached_after"] == 0 and r["resident_after"] == 0 and r["evict"] == 0)]
+        got = [(int(i), int(d), int(c), int(f & 1)) for i, d, c, f in zip(st["id"], st["d"], st["cached"], st["flags"])]
+        assert sorted(got) == sorted(live), f"iteration {it}"
+        assert [x[0] for x in got] == [x[0] for x in live], f"iteration {it}: stored order is the priority order"
+
+
+# ------------------------------------------------------------------------------------------ memory pressure
+
+@pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS])
+@pytest.mark.parametrize("preempt", [W.PRE_RECOMPUTE, W.PRE_SWAP, W.PRE_AUTO])
+def test_pressure_policies_preemption(gpu, oracle_mod, policy, preempt):
+    for seed in range(4):
+        wl = pressure_workload(seed, n=120, kv_blocks=40, policy=policy, preempt=preempt,
+                               guard=1 if policy == W.POLICY_BOOST else 0, swap_pool_blocks=24)
+        g, o = _pair(gpu, oracle_mod, wl)
+        g.run(); o.run()
+        _assert_same(g, o, f"pressure seed {seed} policy {policy} preempt {preempt}")
+        _assert_hist_same(g, o, [0])
+        assert o.stats()[0]["evict_recompute"] + o.stats()[0]["evict_swap"] > 0, "the case must exercise eviction"
+
+
+@pytest.mark.parametrize("signal,quant", [(W.SIG_UNIFIED, W.QUANT_GEOMETRIC), (W.SIG_PHASE, W.QUANT_GEOMETRIC),
+                                          (W.SIG_REMAINING, W.QUANT_EXACT), (W.SIG_UNIFIED, W.QUANT_EXACT)])
+@pytest.mark.parametrize("gamma", [1e-7, 0.05, 0.3, 50.0])
+def test_pressure_signal_quant_gamma(gpu, oracle_mod, signal, quant, gamma):
+    wl = pressure_workload(7, n=150, kv_blocks=56, gamma=gamma, signal=signal, quant=quant, preempt=W.PRE_AUTO,
+                           swap_pool_blocks=30, bin_tokens=32)
+    g, o = _pair(gpu, oracle_mod, wl)
+    g.run(); o.run()
+    _assert_same(g, o, f"signal {signal} quant {quant} gamma {gamma}")
+
+
+def test_step_by_step_under_pressure(gpu, oracle_mod):
+    wl = pressure_workload(3, n=200, kv_blocks=64, preempt=W.PRE_AUTO, swap_pool_blocks=20, mean_gap_us=3000)
+    g, o = _pair(gpu, oracle_mod, wl)
+    for it in range(2500):
+        g.step(1)
+        info, rows = o.step_replica(0)
+        assert g.digest()[0] == o.digest()[0], f"iteration {it}"
+        if not info["executed"]:
+            break
+        st = g.debug_state(0)
+        assert st["clock_us"] == info["t_end_us"]
+        kv = int(sum(-(-int(c) // 16) for c, f in zip(st["cached"], st["flags"]) if f & 1))
+        assert kv == info["kv_resident_after"] <= 64
+
+
+def test_many_replicas_batch_and_granularity(gpu, oracle_mod):
+    """P14: a replica's result does not depend on the batch around it nor on ub_step granularity / iterations per launch."""
+    rng = np.random.default_rng(5)
+    n, NT = 90, 6
+    P = rng.integers(1, 300, (NT, n)); D = rng.integers(1, 200, (NT, n))
+    a = np.cumsum(rng.exponential(6000, (NT, n)), axis=1).astype(np.int64)
+    R = 24
+    rep = W.make_replicas(R, trace_id=np.arange(R) % NT, policy=np.array([0, 1, 2, 3])[np.arange(R) % 4],
+                          gamma=10.0 ** rng.uniform(-2, 1, R), guard=np.arange(R) % 2,
+                          hysteresis_us=rng.integers(0, 200_000, R))
+    sim = dict(kv_blocks=48, queue_cap=64, preempt_mode=W.PRE_AUTO, swap_pool_blocks=16, bin_tokens=64,
+               max_batch=12, chunk_tokens=48, token_budget=80)
+    wl = W.custom(a, P, D, sim, rep)
+    g, o = _pair(gpu, oracle_mod, wl)
+    g.run(); o.run()
+    _assert_same(g, o, "batch of 24")
+    ref = g.digest().copy()
+    g2 = gpu.Sim(wl.sim, wl.replicas, wl.traces(), iters_per_launch=7)
+    for k in (1, 2, 3, 50, 1000, 100000):
+        g2.step(k)
+    assert g2.step(1, want_live=True) == 0
+    assert np.array_equal(g2.digest(), ref)
+    sub = wl.select([23, 5, 11])
+    g3 = gpu.Sim(sub.sim, sub.replicas, sub.traces(), iters_per_launch=64)
+    g3.run()
+    assert np.array_equal(g3.digest(), ref[[23, 5, 11]])
+
+
+# ------------------------------------------------------------------------------------------ edge cases
+
+def test_edge_cases(gpu, oracle_mod):
+    # one request; one token each; identical arrivals (tie-break by id); queue cap smaller than the burst
+    cases = [
+        (np.array([5]), np.array([1]), np.array([1]), {}),
+        (np.zeros(50, np.int64), np.full(50, 3), np.full(50, 2), dict(queue_cap=7, max_batch=3)),
+        (np.arange(40) * 10, np.full(40, 17), np.ones(40, int), dict(kv_blocks=4, chunk_tokens=5, token_budget=9)),
+        (np.zeros(300, np.int64), np.full(300, 40), np.full(300, 30), dict(kv_blocks=30, queue_cap=300, max_batch=300)),
+    ]
+    for i, (a, P, D, kw) in enumerate(cases):
+        sim = dict(kv_blocks=16, preempt_mode=W.PRE_RECOMPUTE)
+        sim.update(kw)
+        wl = W.custom(a, P, D, sim, W.make_replicas(1, trace_id=0))
+        g, o = _pair(gpu, oracle_mod, wl)
+        g.run(); o.run()
+        _assert_same(g, o, f"edge case {i}")
+    # a replica whose trace is empty is done at once
+    wl = W.custom(np.array([[1, 2, 3], [4, 5, 6]]), np.full((2, 3), 4), np.full((2, 3), 2), dict(kv_blocks=8),
+                  W.make_replicas(2))
+    tr = list(wl.traces()); tr[3] = np.array([0, 3], np.uint32)
+    g = gpu.Sim(wl.sim, wl.replicas, tr); o = oracle_mod.OracleSim(wl.sim, wl.replicas, tr)
+    assert g.run() is not None
+    o.run()
+    _assert_same(g, o, "empty trace")
+
+
+def test_full_queue_2048(gpu, oracle_mod):
+    """Maximum queue size: 2048 simultaneously active requests (several sort / scan tiles and a ragged tail)."""
+    n = 2300
+    rng = np.random.default_rng(11)
+    a = np.sort(rng.integers(0, 2000, n)).astype(np.int64)
+    P = rng.integers(1, 64, n); D = rng.integers(1, 12, n)
+    sim = dict(kv_blocks=600, queue_cap=2048, preempt_mode=W.PRE_AUTO, swap_pool_blocks=100, bin_tokens=16,
+               max_batch=256, chunk_tokens=32, token_budget=512)
+    rep = W.make_replicas(3, trace_id=0, policy=[W.POLICY_BOOST, W.POLICY_SRPT, W.POLICY_FCFS], gamma=0.5)
+    wl = W.custom(a, P, D, sim, rep)
+    g, o = _pair(gpu, oracle_mod, wl, ipl=16)
+    g.run(); o.run()
+    _assert_same(g, o, "queue 2048")
+    assert max(s["peak_active"] for s in o.stats()) == 2048
+
+
+def test_load_errors(gpu):
+    from paper_2606_18431_b200 import binding as Bn
+    wl = pressure_workload(0, n=10)
+    a, p, d, n = wl.traces()
+
+    def load(a, p, d, n):
+        h = Bn.ub_create(Bn.make_config(wl.sim))
+        try:
+            return Bn.lib().ub_load_trace(h, np.ascontiguousarray(a, np.int64).ctypes.data,
+                                          np.ascontiguousarray(p, np.int32).ctypes.data,
+                                          np.ascontiguousarray(d, np.int32).ctypes.data,
+                                          np.ascontiguousarray(n, np.uint32).ctypes.data, 0)
+        finally:
+            Bn.ub_destroy(h)
+
+    assert load(a, p, d, n) == Bn.UB_OK
+    a2 = a.copy(); a2[0, 5] = a2[0, 4] - 1
+    assert load(a2, p, d, n) == Bn.UB_EUNSORTED
+    p2 = p.copy(); p2[0, 3] = 0
+    assert load(a, p2, d, n) == Bn.UB_EINFEASIBLE
+    d2 = d.copy(); d2[0, 3] = 10 ** 6
+    assert load(a, p, d2, n) == Bn.UB_EINFEASIBLE
+    a3 = a.copy(); a3[0, 0] = -1
+    assert load(a3, p, d, n) == Bn.UB_EINVAL
+    h = Bn.ub_create(Bn.make_config(wl.sim))
+    assert Bn.lib().ub_step(h, 1, None) == Bn.UB_ESTATE
+    Bn.ub_destroy(h)
+    bad = Bn.make_config(dict(wl.sim, queue_cap=4096))
+    hh = Bn.C.c_void_p()
+    assert Bn.lib().ub_create(Bn.C.byref(bad), Bn.C.byref(hh)) == Bn.UB_EINVAL
+
+
+# ------------------------------------------------------------------------------------------ configs 2-5, sampled replicas
+
+@pytest.mark.parametrize("cfg_id,kw,picks", [
+    (2, dict(n_seeds=4), None),                     # 4 seeds x {FCFS, SRPT, BOOST} = 12 replicas, full run
+    (3, dict(n_seeds=3), None),                     # reasoning mix, MMPP-2, swap-vs-recompute
+    (4, dict(n_seeds=1, n_gamma=16), [0, 5, 9, 15]),  # shift + pressure, 4 of the 16 gamma points
+    (5, dict(n_seeds=2, n_requests=8192), None),    # scale-stress shape, 2 replicas x 8192 requests
+    (6, dict(n_seeds=2), None),                     # starvation shape of PAPER.md:545
+])
+def test_configs_sampled_full_run(gpu, oracle_mod, cfg_id, kw, picks):
+    wl = W.by_id(cfg_id, **kw)
+    if picks is not None:
+        wl = wl.select(picks)
+    g, o = _pair(gpu, oracle_mod, wl, ipl=64)
+    g.run(); o.run()
+    _assert_same(g, o, wl.name)
+    _assert_hist_same(g, o, range(wl.R))
+    assert all(s["done"] == 1 for s in g.stats())
