@@ -24,6 +24,7 @@ struct ub_sim {
   Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; RepPar* d_par; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
   int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
+  uint32_t* d_list; uint32_t* d_count; uint32_t parity;   // work lists [2][4][R], counts [2][4]
   unsigned long long* h_word;            // pinned
   std::vector<uint32_t> h_nreq, h_maxsig;
   std::vector<ub_replica> h_reps;
@@ -86,7 +87,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
       (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
-      (rc = dmalloc(&s->d_word, 2))) {
+      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 8 * R)) || (rc = dmalloc(&s->d_count, 8))) {
     ub_destroy(s);
     return rc;
   }
@@ -116,6 +117,7 @@ void ub_destroy(ub_sim* s) {
   cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_par); cudaFree(s->d_TR);
   cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
+  cudaFree(s->d_list); cudaFree(s->d_count);
   if (s->h_word) cudaFreeHost(s->h_word);
   if (s->ev0) cudaEventDestroy(s->ev0);
   if (s->ev1) cudaEventDestroy(s->ev1);
@@ -261,7 +263,8 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   CK(cudaMemsetAsync(s->d_ne, 0, R * N * 4, s->stream));
   CK(cudaMemsetAsync(s->d_neu, 0, R * N * 4, s->stream));
   CK(cudaMemsetAsync(s->d_hist, 0, R * (size_t)kTbtBins * 4, s->stream));
-  launch_reset(s->dev, s->stream);
+  launch_reset(s->dev, s->d_list, s->d_count, s->stream);
+  s->parity = 0;
   CK(cudaStreamSynchronize(s->stream));
   CK(cudaGetLastError());
   s->have_reps = true;
@@ -273,7 +276,8 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
   uint32_t nl = 0;
   while (n_iters > 0) {
     const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
-    launch_step(s->dev, k, s->stream);
+    launch_step(s->dev, s->d_list, s->d_count, s->parity, k, s->stream);
+    s->parity ^= 1u;
     n_iters -= k; nl++;
   }
   *launches = nl;
@@ -281,7 +285,7 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
 }
 
 static int read_live(ub_sim* s, uint64_t* live) {
-  launch_count_live(s->dev, s->d_word, s->stream);
+  launch_count_live(s->d_count, s->parity, s->d_word, s->stream);
   CK(cudaMemcpyAsync(s->h_word, s->d_word, 8, cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
   CK(cudaGetLastError());

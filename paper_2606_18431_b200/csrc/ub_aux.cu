@@ -38,31 +38,28 @@ void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, 
 }
 
 // ------------------------------------------------------------------ reset (ub_set_replicas)
-__global__ void k_reset(SimDev s) {
+__global__ void k_reset(SimDev s, uint32_t* list, uint32_t* count) {
   const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r == 0) { for (int i = 0; i < 8; i++) count[i] = 0; count[0] = s.R; }    // everybody starts in the S list
   if (r >= s.R) return;
+  list[r] = r;
   Hdr h;
   memset(&h, 0, sizeof(h));
   const uint32_t tr = s.par[r].trace_id;
   h.a_next = (s.n_req[tr] > 0) ? s.TR[(size_t)tr * s.N].a : kNever;
   s.hdr[r] = h;
 }
-void launch_reset(const SimDev& s, cudaStream_t st) { k_reset<<<(s.R + 127) / 128, 128, 0, st>>>(s); }
+void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st) {
+  k_reset<<<(s.R + 127) / 128, 128, 0, st>>>(s, list, count);
+}
 
 // ------------------------------------------------------------------ live replicas (ub_step / ub_run)
-__global__ void k_count_live(SimDev s, unsigned long long* live) {
-  const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
-  int alive = 0;
-  if (r < s.R) {
-    const Hdr* h = s.hdr + r;
-    alive = !(h->n_active == 0 && h->next >= s.n_req[s.par[r].trace_id]);
-  }
-  const int c = __syncthreads_count(alive);
-  if (threadIdx.x == 0 && c) atomicAdd(live, (unsigned long long)c);
+// = the replicas queued in the three work lists the next round consumes
+__global__ void k_count_live(const uint32_t* count, uint32_t parity, unsigned long long* live) {
+  *live = (unsigned long long)count[parity * 4 + 0] + count[parity * 4 + 1] + count[parity * 4 + 2];
 }
-void launch_count_live(const SimDev& s, unsigned long long* live, cudaStream_t st) {
-  cudaMemsetAsync(live, 0, sizeof(unsigned long long), st);
-  k_count_live<<<(s.R + 255) / 256, 256, 0, st>>>(s, live);
+void launch_count_live(const uint32_t* count, uint32_t parity, unsigned long long* live, cudaStream_t st) {
+  k_count_live<<<1, 1, 0, st>>>(count, parity, live);
 }
 
 // ------------------------------------------------------------------ t_last flush (ub_per_request)

@@ -69,13 +69,13 @@ struct SimDev {                 // kernel argument (by value)
 };
 
 // kernels (ub_step.cu, ub_aux.cu)
-void launch_step(const SimDev& s, uint32_t iters, cudaStream_t st);
+void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t parity, uint32_t iters, cudaStream_t st);
 size_t step_smem_bytes(uint32_t Q);
 int  step_configure(uint32_t Q);
 void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
                           uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st);
-void launch_reset(const SimDev& s, cudaStream_t st);
-void launch_count_live(const SimDev& s, unsigned long long* live, cudaStream_t st);
+void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st);
+void launch_count_live(const uint32_t* count, uint32_t parity, unsigned long long* live, cudaStream_t st);
 void launch_flush_tlast(const SimDev& s, cudaStream_t st);
 struct StatsDev {               // device-side result of the percentile reduction, one per replica
   int64_t ttft[3], ttlt[3], tbt[3];
