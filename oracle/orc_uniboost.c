@@ -100,18 +100,24 @@ int64_t orc_tbt_edge(int64_t idx) {
   return (idx - 128 * s) << s;
 }
 
-static uint64_t splitmix64(uint64_t x) {
-  x += 0x9E3779B97F4A7C15ull;
-  uint64_t z = x;
-  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
-  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
-  return z ^ (z >> 31);
-}
-/* M12 event hash: cheap, summed commutatively inside an iteration. */
+/* M12 (test plumbing, not part of the paper's method).  Event hash: a 32-bit mix of
+ * (id, type) times the odd number 2*payload+1.  Inside an iteration the low and the high 32-bit halves of the
+ * event hashes are summed separately, each modulo 2^32 (order-free), and the iteration is folded into H by one
+ * multiply-xorshift round together with t_end. */
 enum { EV_ADMIT = 1, EV_EVICT_RECOMPUTE = 2, EV_EVICT_SWAP = 3, EV_SWAPIN = 4, EV_EMIT_FIRST = 5, EV_COMPLETE = 6 };
-static uint64_t event_hash(uint32_t type, uint32_t id, uint32_t payload) {
-  uint32_t h = ((id + 1u) * 0x9E3779B1u) ^ (type * 0x85EBCA6Bu);
-  return (uint64_t)h * (uint64_t)(uint32_t)(2u * payload + 1u);
+typedef struct { uint32_t lo, hi; } ev_acc;
+static void ev_add(ev_acc* e, uint32_t type, uint32_t id, uint32_t payload) {
+  uint32_t m = ((id + 1u) * 0x9E3779B1u) ^ (type * 0x85EBCA6Bu);
+  uint64_t h = (uint64_t)m * (uint64_t)(uint32_t)(2u * payload + 1u);
+  e->lo += (uint32_t)h;
+  e->hi += (uint32_t)(h >> 32);
+}
+static uint64_t digest_fold(uint64_t H, ev_acc e, int64_t t_end) {
+  uint64_t x = (H ^ (((uint64_t)e.hi << 32) | (uint64_t)e.lo)) + (uint64_t)t_end * 0x9E3779B97F4A7C15ull;
+  x ^= x >> 29;
+  x *= 0xBF58476D1CE4E5B9ull;
+  x ^= x >> 32;
+  return x;
 }
 
 const char* orc_strerror(int e) {
@@ -308,7 +314,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
   /* M7 admission walk: B <- {}, U <- claims; while |B| < M ... */
   int64_t C = 0, tok = 0, cnt = 0, newblocked = 0;
   int64_t prefill_tokens = 0, decode_seqs = 0, swap_blocks = 0;
-  uint64_t ev = 0;
+  ev_acc ev = {0u, 0u};
   for (int64_t j = 0; j < n; j++) {
     if (cnt == c->max_batch || tok == c->token_budget) break;
     orc_req* q = &x->req[e[j].id];
@@ -325,11 +331,11 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
     }
     e[j].want = want; C += foot; tok += want; cnt++;
     if (q->d >= 1 && rem == 1) decode_seqs++; else prefill_tokens += want;   /* M9 */
-    ev += event_hash(EV_ADMIT, (uint32_t)e[j].id, (uint32_t)want);
+    ev_add(&ev, EV_ADMIT, (uint32_t)e[j].id, (uint32_t)want);
     if (q->swapped) {                                    /* swap-in on admission (M9) */
       int64_t blocks = ceil_div(q->cached, blk);
       swap_blocks += blocks; x->swap_used -= blocks; x->swapins++;
-      ev += event_hash(EV_SWAPIN, (uint32_t)e[j].id, (uint32_t)blocks);
+      ev_add(&ev, EV_SWAPIN, (uint32_t)e[j].id, (uint32_t)blocks);
     }
   }
 
@@ -349,11 +355,11 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
                 (2 * res * c->swap_ns_per_block < 1000 * c->c_prefill_tok_us * (int64_t)q->cached);
     if (do_swap) {
       q->swapped = 1; x->swap_used += res; swap_blocks += res; x->evict_swap++;
-      ev += event_hash(EV_EVICT_SWAP, (uint32_t)e[j].id, (uint32_t)res);
+      ev_add(&ev, EV_EVICT_SWAP, (uint32_t)e[j].id, (uint32_t)res);
       e[j].evict = 2;
     } else {
       x->tokens_lost += q->cached;
-      ev += event_hash(EV_EVICT_RECOMPUTE, (uint32_t)e[j].id, (uint32_t)q->cached);
+      ev_add(&ev, EV_EVICT_RECOMPUTE, (uint32_t)e[j].id, (uint32_t)q->cached);
       q->cached = 0; x->evict_recompute++;
       e[j].evict = 1;
     }
@@ -376,7 +382,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
     q->resident = 1; q->swapped = 0; q->cached += (int32_t)e[j].want;
     if (q->cached == Pp[id] + q->d) {
       q->d++; x->tokens_emitted++;
-      if (q->d == 1) { q->t_first = t_end; ev += event_hash(EV_EMIT_FIRST, (uint32_t)id, 0); }
+      if (q->d == 1) { q->t_first = t_end; ev_add(&ev, EV_EMIT_FIRST, (uint32_t)id, 0); }
       else x->hist[orc_tbt_bin(t_end - q->t_last)]++;
       q->t_last = t_end;
       if (q->d == Dd[id]) {
@@ -384,7 +390,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
         x->n_completed++;
         x->sum_ttft += q->t_first - A[id]; x->sum_ttlt += q->t_last - A[id];
         x->sum_tbt_num += q->t_last - q->t_first; x->sum_tbt_den += Dd[id] - 1;
-        ev += event_hash(EV_COMPLETE, (uint32_t)id, 0);
+        ev_add(&ev, EV_COMPLETE, (uint32_t)id, 0);
       }
     }
   }
@@ -401,7 +407,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
   x->n_active = m;
 
   /* M12 digest */
-  x->H = splitmix64(x->H ^ ev ^ splitmix64((uint64_t)t_end));
+  x->H = digest_fold(x->H, ev, t_end);
   x->iterations++; x->request_steps += n;
   x->prefill_tokens += prefill_tokens; x->decode_seqs += decode_seqs;
 

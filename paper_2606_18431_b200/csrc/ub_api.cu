@@ -24,7 +24,7 @@ struct ub_sim {
   Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; RepPar* d_par; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
   int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
-  uint32_t* d_list; uint32_t* d_count; uint32_t parity;   // work lists [2][4][R], counts [2][4]
+  uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([4] = finished replicas)
   unsigned long long* h_word;            // pinned
   std::vector<uint32_t> h_nreq, h_maxsig;
   std::vector<ub_replica> h_reps;
@@ -87,7 +87,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
       (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
-      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 8 * R)) || (rc = dmalloc(&s->d_count, 8))) {
+      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 4 * R)) || (rc = dmalloc(&s->d_count, 8))) {
     ub_destroy(s);
     return rc;
   }
@@ -101,6 +101,8 @@ int ub_create(const ub_config* c, ub_sim** out) {
   SimDev& d = s->dev;
   memset(&d, 0, sizeof(d));
   d.R = c->n_replicas; d.NT = c->n_traces; d.N = c->max_requests; d.Q = c->queue_cap;
+  d.blk_shift = 32;
+  for (uint32_t b = 0; b < 32; b++) if ((1u << b) == c->block_tokens) d.blk_shift = b;
   d.B = c->kv_blocks; d.blk = c->block_tokens; d.M = c->max_batch; d.c = c->chunk_tokens; d.T = c->token_budget;
   d.preempt_mode = c->preempt_mode; d.swap_ns = c->swap_ns_per_block; d.swap_pool = c->swap_pool_blocks;
   d.k = c->bin_tokens; d.c0 = c->c0_us; d.c_pf = c->c_prefill_tok_us; d.c_dec = c->c_decode_seq_us;
@@ -264,7 +266,6 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   CK(cudaMemsetAsync(s->d_neu, 0, R * N * 4, s->stream));
   CK(cudaMemsetAsync(s->d_hist, 0, R * (size_t)kTbtBins * 4, s->stream));
   launch_reset(s->dev, s->d_list, s->d_count, s->stream);
-  s->parity = 0;
   CK(cudaStreamSynchronize(s->stream));
   CK(cudaGetLastError());
   s->have_reps = true;
@@ -276,8 +277,7 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
   uint32_t nl = 0;
   while (n_iters > 0) {
     const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
-    launch_step(s->dev, s->d_list, s->d_count, s->parity, k, s->stream);
-    s->parity ^= 1u;
+    launch_step(s->dev, s->d_list, s->d_count, k, s->stream);
     n_iters -= k; nl++;
   }
   *launches = nl;
@@ -285,7 +285,7 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
 }
 
 static int read_live(ub_sim* s, uint64_t* live) {
-  launch_count_live(s->d_count, s->parity, s->d_word, s->stream);
+  launch_count_live(s->d_count, s->cfg.n_replicas, s->d_word, s->stream);
   CK(cudaMemcpyAsync(s->h_word, s->d_word, 8, cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
   CK(cudaGetLastError());

@@ -38,28 +38,30 @@ void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, 
 }
 
 // ------------------------------------------------------------------ reset (ub_set_replicas)
-__global__ void k_reset(SimDev s, uint32_t* list, uint32_t* count) {
+// count[0..3] = work lists of the current round, count[4] = replicas that have finished their trace
+__global__ void k_reset(SimDev s, uint32_t* count) {
   const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
-  if (r == 0) { for (int i = 0; i < 8; i++) count[i] = 0; count[0] = s.R; }    // everybody starts in the S list
   if (r >= s.R) return;
-  list[r] = r;
   Hdr h;
   memset(&h, 0, sizeof(h));
   const uint32_t tr = s.par[r].trace_id;
-  h.a_next = (s.n_req[tr] > 0) ? s.TR[(size_t)tr * s.N].a : kNever;
+  const bool empty = s.n_req[tr] == 0;
+  h.a_next = empty ? kNever : s.TR[(size_t)tr * s.N].a;
   s.hdr[r] = h;
+  if (empty) atomicAdd(count + 4, 1u);
 }
 void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st) {
-  k_reset<<<(s.R + 127) / 128, 128, 0, st>>>(s, list, count);
+  (void)list;
+  cudaMemsetAsync(count, 0, 8 * sizeof(uint32_t), st);
+  k_reset<<<(s.R + 127) / 128, 128, 0, st>>>(s, count);
 }
 
 // ------------------------------------------------------------------ live replicas (ub_step / ub_run)
-// = the replicas queued in the three work lists the next round consumes
-__global__ void k_count_live(const uint32_t* count, uint32_t parity, unsigned long long* live) {
-  *live = (unsigned long long)count[parity * 4 + 0] + count[parity * 4 + 1] + count[parity * 4 + 2];
+__global__ void k_count_live(const uint32_t* count, uint32_t R, unsigned long long* live) {
+  *live = (unsigned long long)(R - count[4]);
 }
-void launch_count_live(const uint32_t* count, uint32_t parity, unsigned long long* live, cudaStream_t st) {
-  k_count_live<<<1, 1, 0, st>>>(count, parity, live);
+void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* live, cudaStream_t st) {
+  k_count_live<<<1, 1, 0, st>>>(count, R, live);
 }
 
 // ------------------------------------------------------------------ t_last flush (ub_per_request)

@@ -5,7 +5,7 @@
 // arrays kept in PRIORITY ORDER of the last executed iteration (so the next iteration finds it nearly sorted):
 //   E0[r][Q] = { a: i64 arrival us, P: u32 prompt tokens, D: u32 hidden output tokens }   static per request
 //   E1[r][Q] = { id: u32, d: u32 tokens emitted, cached: u32 KV tokens held, flags: u32 } dynamic
-// plus one 160-byte header Hdr[r], the packed traces TR[trace][N] (same 16-byte record as E0), the
+// plus one 160-byte header Hdr[r] (8-byte word i is addressed directly by the fast kernel: keep the order), the packed traces TR[trace][N] (same 16-byte record as E0), the
 // per-request outputs t_first/t_last/n_evict/n_evict_unforced [R][N] and the TBT histogram [R][4352].
 #pragma once
 #include <cuda_runtime.h>
@@ -55,6 +55,7 @@ struct SimDev {                 // kernel argument (by value)
   // configuration
   uint32_t R, NT, N, Q;
   uint32_t B, blk, M, c, T;
+  uint32_t blk_shift;           // log2(blk) if blk is a power of two, else 32
   uint32_t preempt_mode, swap_ns, swap_pool, k;
   int64_t  c0, c_pf, c_dec;
   // state
@@ -69,13 +70,15 @@ struct SimDev {                 // kernel argument (by value)
 };
 
 // kernels (ub_step.cu, ub_aux.cu)
-void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t parity, uint32_t iters, cudaStream_t st);
+void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, cudaStream_t st);
+void launch_fast(const struct StepArgs& A, cudaStream_t st);      // ub_fast.cu
+int  fast_configure();
 size_t step_smem_bytes(uint32_t Q);
 int  step_configure(uint32_t Q);
 void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
                           uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st);
 void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st);
-void launch_count_live(const uint32_t* count, uint32_t parity, unsigned long long* live, cudaStream_t st);
+void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* live, cudaStream_t st);
 void launch_flush_tlast(const SimDev& s, cudaStream_t st);
 struct StatsDev {               // device-side result of the percentile reduction, one per replica
   int64_t ttft[3], ttlt[3], tbt[3];

@@ -13,63 +13,12 @@
 // the exchange buffer of the ordering step.  Replicas are binned by window size into three work lists
 // (S: one warp per replica, M: 4 warps, L: 8 warps) that the kernels of iteration i build for iteration i+1.
 // Integer arithmetic only.
-#include "ub_internal.cuh"
+#include "ub_device.cuh"
 
 namespace ub {
 
 // ---------------------------------------------------------------------------------------------- helpers
 
-__device__ __forceinline__ uint32_t ceil_div_u32(uint32_t x, uint32_t y) { return (x + y - 1) / y; }
-
-__device__ __forceinline__ uint64_t splitmix64(uint64_t x) {
-  x += 0x9E3779B97F4A7C15ull;
-  uint64_t z = x;
-  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
-  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
-  return z ^ (z >> 31);
-}
-
-// M12 event hash; events are summed (wrapping) inside an iteration, so the reduction order is free.
-enum { EV_ADMIT = 1, EV_EVICT_RECOMPUTE = 2, EV_EVICT_SWAP = 3, EV_SWAPIN = 4, EV_EMIT_FIRST = 5, EV_COMPLETE = 6 };
-__device__ __forceinline__ uint64_t event_hash(uint32_t type, uint32_t id, uint32_t payload) {
-  uint32_t h = ((id + 1u) * 0x9E3779B1u) ^ (type * 0x85EBCA6Bu);
-  return (uint64_t)h * (uint64_t)(2u * payload + 1u);
-}
-
-// M11 log-linear bin of a TBT gap (7 sub-bits).
-__device__ __forceinline__ uint32_t tbt_bin(int64_t g) {
-  if (g < 0) g = 0;
-  if (g >= ((int64_t)1 << 40)) g = ((int64_t)1 << 40) - 1;
-  int lg = (g > 0) ? 63 - __clzll((long long)g) : 0;
-  int shift = lg - 7; if (shift < 0) shift = 0;
-  return (uint32_t)(128 * shift + (g >> shift));
-}
-
-// Eq. 8 exponent: floor(log2(max(sig,k)/k)) == largest b with k 2^b <= max(sig,k)  (sig, k < 2^31)
-__device__ __forceinline__ uint32_t geo_bin(uint32_t sig, uint32_t k) {
-  uint32_t s = sig > k ? sig : k;
-  int b = __clz(k) - __clz(s);
-  if (((uint64_t)k << b) > (uint64_t)s) b--;
-  return (uint32_t)b;
-}
-
-__device__ __forceinline__ uint32_t signal_of(const RepPar& par, uint32_t P, uint32_t D, uint32_t d) {
-  if (par.signal_mode == 0) return P + d;                       // w~ = max(w, s_pre)
-  if (par.signal_mode == 1) return (d == 0) ? P : d;            // SIGNAL
-  return D - d;                                                 // remaining (tests: SRPT limit)
-}
-__device__ __forceinline__ uint32_t bin_of(const RepPar& par, uint32_t k, uint32_t sig) {
-  return (par.quant_mode == 0) ? geo_bin(sig, k) : sig;         // QUANTIZE, Eq. 8
-}
-
-__device__ __forceinline__ uint32_t warp_scan_incl(uint32_t v, int lane) {
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    uint32_t n = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= o) v += n;
-  }
-  return v;
-}
 __device__ __forceinline__ uint64_t warp_sum_u64(uint64_t v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -78,9 +27,6 @@ __device__ __forceinline__ uint64_t warp_sum_u64(uint64_t v) {
 
 // ordering record in the exchange buffer: (okey, id) is the total order; aux carries the dirty hint
 struct __align__(16) KeyRec { uint64_t okey; uint32_t id; uint32_t aux; };
-__device__ __forceinline__ bool key_less(uint64_t ka, uint32_t ia, uint64_t kb, uint32_t ib) {
-  return ka < kb || (ka == kb && ia < ib);
-}
 
 // ---------------------------------------------------------------------------------------------- team primitives
 // WARPS == 1: a team is a warp, everything is shuffles.  WARPS > 1: the team is the whole CTA.
@@ -159,21 +105,6 @@ template <int WARPS> struct Team {
   }
 };
 
-// ---------------------------------------------------------------------------------------------- work lists
-// list[(parity*4 + cls) * R + i], count[parity*4 + cls]; cls 0 = S, 1 = M, 2 = L, 3 = overflow of this iteration.
-
-struct StepArgs {
-  SimDev s;
-  uint32_t* list; uint32_t* count;
-  uint32_t parity, iters;
-  uint32_t thrS, thrM;          // window size up to which a replica is queued for the S / M kernel
-};
-
-__device__ __forceinline__ void push_list(const StepArgs& A, uint32_t slot, uint32_t r) {
-  const uint32_t idx = atomicAdd(A.count + slot, 1u);
-  A.list[(size_t)slot * A.s.R + idx] = r;
-}
-
 // ---------------------------------------------------------------------------------------------- one replica, `iters` iterations
 
 template <int WARPS, int E>
@@ -202,7 +133,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
   uint32_t* g_hist = s.hist + (size_t)r * kTbtBins;
   uint32_t* g_ne = s.n_evict + (size_t)r * s.N;          // bit 31 = completed marker (read by the stats kernel)
   uint32_t* g_neu = s.n_evict_unf + (size_t)r * s.N;
-  const uint32_t B = s.B, blk = s.blk, M = s.M, cc = s.c, Tb = s.T, Q = s.Q;
+  const uint32_t B = s.B, M = s.M, cc = s.c, Tb = s.T, Q = s.Q;
 
   // ---- header: thread i < 20 of warp 0 holds 64-bit word i of Hdr
   uint64_t* ghdr = reinterpret_cast<uint64_t*>(s.hdr + r);
@@ -230,7 +161,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
     __syncthreads();
   }
   const uint32_t iters = todo ? todo : A.iters;
-  bool handed_over = false;
+  bool handed_over = false, ran = false;
 
   for (uint32_t it = 0; it < iters; it++) {
     // ---------------- a0: idle jump + ingest (M6)
@@ -460,7 +391,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
           const uint32_t tok_before = (W - w) < Tb ? (W - w) : Tb;
           const uint32_t tok_after = W < Tb ? W : Tb;
           const uint32_t wnt = tok_after - tok_before;
-          const uint32_t foot = valid ? ceil_div_u32(r1[c].cached + wnt, blk) : 0u;
+          const uint32_t foot = valid ? blocks_of(s, r1[c].cached + wnt) : 0u;
           const uint32_t Cf = carryC + tm.scan_incl(foot, ctot);
           uint32_t cnt_before;
           if (only_res) {
@@ -509,7 +440,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
 
     // ---------------- a4: batch totals (M9) and victim select (M8; SELECTVICTIM / SWAPOUT)
     uint32_t tot5[5] = {0, 0, 0, 0, 0};          // prefill tokens, decode seqs, swap-in blocks, swap-ins, K blocks
-    uint64_t evh = 0;
+    uint32_t evl = 0, evu = 0;                   // M12: low / high halves of the event hashes, summed mod 2^32
 #pragma unroll
     for (int c = 0; c < E; c++) {
       const uint32_t pos = c * TH + tid;
@@ -517,19 +448,20 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         if (want[c]) {
           const uint32_t rem = r0[c].P + r1[c].d - r1[c].cached;
           if (r1[c].d >= 1 && rem == 1) tot5[1]++; else tot5[0] += want[c];       // decode sequence vs prefill tokens
-          evh += event_hash(EV_ADMIT, r1[c].id, want[c]);
+          ev_add(evl, evu, EV_ADMIT, r1[c].id, want[c]);
           if (r1[c].flags & F_SWAPPED) {                                          // swap-in on admission
-            const uint32_t blocks = ceil_div_u32(r1[c].cached, blk);
+            const uint32_t blocks = blocks_of(s, r1[c].cached);
             tot5[2] += blocks; tot5[3]++;
-            evh += event_hash(EV_SWAPIN, r1[c].id, blocks);
+            ev_add(evl, evu, EV_SWAPIN, r1[c].id, blocks);
           }
         } else if (r1[c].flags & F_RESIDENT) {
-          tot5[4] += ceil_div_u32(r1[c].cached, blk);                             // non-admitted resident keeps its blocks
+          tot5[4] += blocks_of(s, r1[c].cached);                             // non-admitted resident keeps its blocks
         }
       }
     }
     tm.template sum32<5>(tot5);
-    uint64_t ev_tot = tm.sum64(evh);
+    uint32_t ev2[2] = {evl, evu};
+    tm.template sum32<2>(ev2);
     const uint32_t pf_tot = tot5[0], dec_tot = tot5[1], swin_blocks = tot5[2], swin_cnt = tot5[3], kres_tot = tot5[4];
     swap_used -= swin_blocks;
     uint32_t swout_blocks = 0, ev_nsw = 0, ev_nrc = 0;
@@ -546,7 +478,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
       for (int c = 0; c < E; c++) {
         const uint32_t pos = c * TH + tid;
         uint32_t v = 0;
-        if (pos < n && want[c] == 0 && (r1[c].flags & F_RESIDENT)) v = ceil_div_u32(r1[c].cached, blk);
+        if (pos < n && want[c] == 0 && (r1[c].flags & F_RESIDENT)) v = blocks_of(s, r1[c].cached);
         uint32_t tot, etot;
         const uint32_t ps = carry + tm.scan_incl(v, tot);
         mine[c] = (v > 0) && ps > thr;           // a resident holds >= 1 block, so v > 0 <=> member of K
@@ -556,25 +488,25 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
       }
       tm.sync();
       if (tid == 0) {                            // lowest priority first; the swap pool is a sequential resource
-        uint32_t su = swap_used, swo = 0, n_sw = 0, n_rc = 0; uint64_t eh = 0, lost = 0;
+        uint32_t su = swap_used, swo = 0, n_sw = 0, n_rc = 0, ehl = 0, ehu = 0; uint64_t lost = 0;
         for (int e = (int)ecarry - 1; e >= 0; e--) {
           const uint4 q = x_ev[e];
-          const uint32_t resb = ceil_div_u32(q.y, blk);
+          const uint32_t resb = blocks_of(s, q.y);
           bool do_swap = false;
           if (s.preempt_mode == 1) do_swap = (su + resb <= s.swap_pool);
           else if (s.preempt_mode == 2)
             do_swap = (su + resb <= s.swap_pool) && (2ll * resb * (int64_t)s.swap_ns < 1000ll * s.c_pf * (int64_t)q.y);
-          if (do_swap) { su += resb; swo += resb; n_sw++; eh += event_hash(EV_EVICT_SWAP, q.x, resb); x_mode[q.w] = 2; }
-          else { lost += q.y; n_rc++; eh += event_hash(EV_EVICT_RECOMPUTE, q.x, q.y); x_mode[q.w] = 1; }
+          if (do_swap) { su += resb; swo += resb; n_sw++; ev_add(ehl, ehu, EV_EVICT_SWAP, q.x, resb); x_mode[q.w] = 2; }
+          else { lost += q.y; n_rc++; ev_add(ehl, ehu, EV_EVICT_RECOMPUTE, q.x, q.y); x_mode[q.w] = 1; }
           g_ne[q.x] = __ldcg(g_ne + q.x) + 1u;
           if (q.z) g_neu[q.x] = __ldcg(g_neu + q.x) + 1u;      // victim was not MemGuard-locked
         }
         ts->bc[8] = su; ts->bc[9] = swo; ts->bc[10] = n_sw; ts->bc[11] = n_rc;
-        ts->bc64[5] = eh; ts->bc64[6] = lost;
+        ts->bc[12] = ehl; ts->bc[13] = ehu; ts->bc64[6] = lost;
       }
       tm.sync();
       swap_used = ts->bc[8]; swout_blocks = ts->bc[9]; ev_nsw = ts->bc[10]; ev_nrc = ts->bc[11];
-      ev_tot += ts->bc64[5]; ev_lost = ts->bc64[6];
+      ev2[0] += ts->bc[12]; ev2[1] += ts->bc[13]; ev_lost = ts->bc64[6];
 #pragma unroll
       for (int c = 0; c < E; c++) if (mine[c]) evm[c] = x_mode[c * TH + tid];
       tm.sync();
@@ -603,7 +535,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
             r1[c].d = d_old + 1; tot2[0]++;
             if (d_old == 0) {
               g_tfirst[id] = t_end;
-              atomicAdd(&ts->acc64[0], (unsigned long long)event_hash(EV_EMIT_FIRST, id, 0));
+              { uint32_t l_ = 0, u_ = 0; ev_add(l_, u_, EV_EMIT_FIRST, id, 0); atomicAdd(&ts->acc32[2], l_); atomicAdd(&ts->acc32[3], u_); }
             } else if (nf & F_EMITPREV) {
               tot2[1]++;                                        // gap == this iteration's cost
             } else {
@@ -618,7 +550,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
               atomicAdd(&ts->acc64[2], (unsigned long long)(t_end - r0[c].a));
               atomicAdd(&ts->acc64[3], (unsigned long long)(t_end - tf));
               atomicAdd(&ts->acc64[4], (unsigned long long)(r0[c].D - 1));
-              atomicAdd(&ts->acc64[0], (unsigned long long)event_hash(EV_COMPLETE, id, 0));
+              { uint32_t l_ = 0, u_ = 0; ev_add(l_, u_, EV_COMPLETE, id, 0); atomicAdd(&ts->acc32[2], l_); atomicAdd(&ts->acc32[3], u_); }
               atomicAdd(&ts->acc32[0], 1u);
               g_ne[id] = __ldcg(g_ne + id) | 0x80000000u;
               gone[c] = true;
@@ -671,12 +603,12 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
     // ---------------- header words (thread i of warp 0 owns word i)
     if (tid == 0 && tot2[1]) atomicAdd(&g_hist[tbt_bin(cost)], tot2[1]);
     {
-      const uint64_t evs = ev_tot + ts->acc64[0];
+      const uint32_t evs_lo = ev2[0] + ts->acc32[2], evs_hi = ev2[1] + ts->acc32[3];
       const uint32_t n_done = ts->acc32[0];
       if (warp == 0) {
         switch (lane) {
           case 0: hv = (uint64_t)t_end; break;
-          case 1: hv = splitmix64(hv ^ evs ^ splitmix64((uint64_t)t_end)); break;
+          case 1: hv = digest_fold(hv, evs_lo, evs_hi, t_end); break;
           case 2: hv = (uint64_t)a_next; break;
           case 3: hv += n; break;
           case 4: hv += tot2[0]; break;
@@ -696,22 +628,18 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         }
       }
     }
-    t = t_end; n = n_new;
+    t = t_end; n = n_new; ran = true;
     tm.sync();                                   // window stores / smem accumulators before the next iteration
   }
 
-  // ---------------- header -> HBM, queue the replica for the next iteration
+  // ---------------- header -> HBM; a window that outgrew this team goes to the overflow list of this round
   if (warp == 0) {
     if (lane == 17) hv = (hv & 0xFFFFFFFFull) | ((uint64_t)(handed_over ? todo : 0u) << 32);
     if (lane < 20) ghdr[lane] = hv;
   }
   if (tid == 0) {
-    if (handed_over) {
-      push_list(A, A.parity * 4 + 3, r);                         // overflow list of THIS iteration
-    } else if (!(n == 0 && next >= nreq)) {
-      const uint32_t cls = n <= A.thrS ? 0u : (n <= A.thrM ? 1u : 2u);
-      push_list(A, (A.parity ^ 1u) * 4 + cls, r);
-    }
+    if (handed_over) push_list(A, 3, r);
+    else if (ran && n == 0 && next >= nreq) atomicAdd(A.count + 4, 1u);      // finished its trace in this call
   }
 }
 
@@ -756,26 +684,28 @@ int step_configure(uint32_t) {
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_step<1, kES, kTeamsS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(kTeamsS * TeamSmem<1, kES>::BYTES));
+  if (e == cudaSuccess) return fast_configure();
   return (int)e;
 }
 
-// One scheduler round (`iters` iterations of every live replica): L list, M list, S list, then the overflow list.
-void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t parity, uint32_t iters, cudaStream_t st) {
+// One scheduler round (`iters` iterations of every live replica): the fast kernel visits every replica and queues
+// what it does not handle (large windows, evictions, re-sorts) for the team kernels: L list, M list, S list, then
+// the overflow list.
+void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, cudaStream_t st) {
   StepArgs A;
-  A.s = s; A.list = list; A.count = count; A.parity = parity; A.iters = iters;
+  A.s = s; A.list = list; A.count = count; A.iters = iters;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
-  cudaMemsetAsync(count + (parity ^ 1u) * 4, 0, 4 * sizeof(uint32_t), st);      // next round's lists start empty
-  cudaMemsetAsync(count + parity * 4 + 3, 0, sizeof(uint32_t), st);             // this round's overflow list
+  cudaMemsetAsync(count, 0, 4 * sizeof(uint32_t), st);                          // this round's lists start empty
+  launch_fast(A, st);
   const uint32_t R = s.R;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;
   const uint32_t nS = (R + kTeamsS - 1) / kTeamsS, gS = nS < 148u * 10 ? nS : 148u * 10;
-  const uint32_t p4 = parity * 4;
-  k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, p4 + 2, 0xFFFFFFFFu);
-  k_step<4, kEM, 1><<<gM, 128, TeamSmem<4, kEM>::BYTES, st>>>(A, p4 + 1, 0xFFFFFFFFu);
-  k_step<1, kES, kTeamsS><<<gS, 32 * kTeamsS, kTeamsS * TeamSmem<1, kES>::BYTES, st>>>(A, p4 + 0, 0xFFFFFFFFu);
-  k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, p4 + 3, 0xFFFFFFFFu);
+  k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 2u, 0xFFFFFFFFu);
+  k_step<4, kEM, 1><<<gM, 128, TeamSmem<4, kEM>::BYTES, st>>>(A, 1u, 0xFFFFFFFFu);
+  k_step<1, kES, kTeamsS><<<gS, 32 * kTeamsS, kTeamsS * TeamSmem<1, kES>::BYTES, st>>>(A, 0u, 0xFFFFFFFFu);
+  k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 3u, 0xFFFFFFFFu);
 }
 
 }  // namespace ub
