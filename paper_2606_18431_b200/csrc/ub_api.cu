@@ -24,7 +24,7 @@ struct ub_sim {
   Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; RepPar* d_par; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
   int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
-  uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([4] = finished replicas)
+  uint32_t* d_list; uint32_t* d_count;   // work lists [5][R]; counts [8] ([5] = finished replicas)
   unsigned long long* h_word;            // pinned
   std::vector<uint32_t> h_nreq, h_maxsig;
   std::vector<ub_replica> h_reps;
@@ -87,7 +87,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
       (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
-      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 4 * R)) || (rc = dmalloc(&s->d_count, 8))) {
+      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 5 * R)) || (rc = dmalloc(&s->d_count, 8))) {
     ub_destroy(s);
     return rc;
   }

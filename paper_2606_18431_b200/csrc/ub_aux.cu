@@ -38,7 +38,7 @@ void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, 
 }
 
 // ------------------------------------------------------------------ reset (ub_set_replicas)
-// count[0..3] = work lists of the current round, count[4] = replicas that have finished their trace
+// count[0..3] = work lists of the current round, count[4] = list of the second lean instance, count[5] = replicas that have finished their trace
 __global__ void k_reset(SimDev s, uint32_t* count) {
   const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= s.R) return;
@@ -48,7 +48,7 @@ __global__ void k_reset(SimDev s, uint32_t* count) {
   const bool empty = s.n_req[tr] == 0;
   h.a_next = empty ? kNever : s.TR[(size_t)tr * s.N].a;
   s.hdr[r] = h;
-  if (empty) atomicAdd(count + 4, 1u);
+  if (empty) atomicAdd(count + 5, 1u);
 }
 void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st) {
   (void)list;
@@ -58,7 +58,7 @@ void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t
 
 // ------------------------------------------------------------------ live replicas (ub_step / ub_run)
 __global__ void k_count_live(const uint32_t* count, uint32_t R, unsigned long long* live) {
-  *live = (unsigned long long)(R - count[4]);
+  *live = (unsigned long long)(R - count[5]);
 }
 void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* live, cudaStream_t st) {
   k_count_live<<<1, 1, 0, st>>>(count, R, live);

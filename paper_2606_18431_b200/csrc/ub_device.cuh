@@ -71,7 +71,8 @@ __device__ __forceinline__ bool key_less(uint64_t ka, uint32_t ia, uint64_t kb, 
 // ---------------------------------------------------------------------------------------------- work lists
 // Per scheduler round: the fast kernel visits every replica and queues the ones it does not handle itself into
 // list[cls * R + i], count[cls]; cls 0 = S (1 warp), 1 = M (4 warps), 2 = L (8 warps), 3 = overflow (a window that
-// outgrew its team during the round).  count[4] = replicas that have finished their trace (monotone).
+// outgrew its team during the round), 4 = windows of 65..128 requests for the second lean instance.
+// count[5] = replicas that have finished their trace (monotone).
 struct StepArgs {
   SimDev s;
   uint32_t* list; uint32_t* count;

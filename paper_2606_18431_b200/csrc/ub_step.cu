@@ -639,7 +639,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
   }
   if (tid == 0) {
     if (handed_over) push_list(A, 3, r);
-    else if (ran && n == 0 && next >= nreq) atomicAdd(A.count + 4, 1u);      // finished its trace in this call
+    else if (ran && n == 0 && next >= nreq) atomicAdd(A.count + 5, 1u);      // finished its trace in this call
   }
 }
 
@@ -697,7 +697,7 @@ void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iter
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
-  cudaMemsetAsync(count, 0, 4 * sizeof(uint32_t), st);                          // this round's lists start empty
+  cudaMemsetAsync(count, 0, 5 * sizeof(uint32_t), st);                          // this round's lists start empty
   launch_fast(A, st);
   const uint32_t R = s.R;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;
