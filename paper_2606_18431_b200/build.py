@@ -8,7 +8,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libuniboost.so")
-SOURCES = ["ub_fast.cu", "ub_step.cu", "ub_aux.cu", "ub_api.cu"]
+SOURCES = ["ub_stream.cu", "ub_step.cu", "ub_aux.cu", "ub_api.cu"]
 HEADERS = [os.path.join(CSRC, "ub_internal.cuh"), os.path.join(CSRC, "ub_device.cuh"), os.path.join(HERE, "..", "include", "uniboost.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

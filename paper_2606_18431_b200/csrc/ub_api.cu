@@ -24,7 +24,8 @@ struct ub_sim {
   Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; RepPar* d_par; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
   int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
-  uint32_t* d_list; uint32_t* d_count;   // work lists [5][R]; counts [8] ([5] = finished replicas)
+  uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([5] = finished replicas)
+  uint16_t* d_dlist; uint2* d_evbuf;     // dirty lists [R][kDirtyMax]; per-iteration event scratch [R][min(M,Q)]
   unsigned long long* h_word;            // pinned
   std::vector<uint32_t> h_nreq, h_maxsig;
   std::vector<ub_replica> h_reps;
@@ -87,7 +88,9 @@ int ub_create(const ub_config* c, ub_sim** out) {
       (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
-      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 5 * R)) || (rc = dmalloc(&s->d_count, 8))) {
+      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 4 * R)) || (rc = dmalloc(&s->d_count, 8)) ||
+      (rc = dmalloc(&s->d_dlist, R * kDirtyMax)) ||
+      (rc = dmalloc(&s->d_evbuf, R * (size_t)(c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap)))) {
     ub_destroy(s);
     return rc;
   }
@@ -107,6 +110,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
   d.preempt_mode = c->preempt_mode; d.swap_ns = c->swap_ns_per_block; d.swap_pool = c->swap_pool_blocks;
   d.k = c->bin_tokens; d.c0 = c->c0_us; d.c_pf = c->c_prefill_tok_us; d.c_dec = c->c_decode_seq_us;
   d.E0 = s->d_E0; d.E1 = s->d_E1; d.hdr = s->d_hdr; d.par = s->d_par; d.n_req = s->d_nreq;
+  d.dlist = s->d_dlist; d.evbuf = s->d_evbuf; d.evcap = c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap;
   d.t_first = s->d_tfirst; d.t_last = s->d_tlast; d.n_evict = s->d_ne; d.n_evict_unf = s->d_neu; d.hist = s->d_hist;
   *out = s;
   return UB_OK;
@@ -119,7 +123,7 @@ void ub_destroy(ub_sim* s) {
   cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_par); cudaFree(s->d_TR);
   cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
-  cudaFree(s->d_list); cudaFree(s->d_count);
+  cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dlist); cudaFree(s->d_evbuf);
   if (s->h_word) cudaFreeHost(s->h_word);
   if (s->ev0) cudaEventDestroy(s->ev0);
   if (s->ev1) cudaEventDestroy(s->ev1);

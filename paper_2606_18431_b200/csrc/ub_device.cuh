@@ -1,4 +1,4 @@
-// ub_device.cuh -- device helpers shared by the step kernels (ub_fast.cu: lean warp-per-replica path,
+// ub_device.cuh -- device helpers shared by the step kernels (ub_stream.cu: streaming warp-per-replica path,
 // ub_step.cu: general team-per-replica path).  Both kernels operate on the same HBM state (ub_internal.cuh),
 // so a replica may be advanced by either one in any iteration.  Nothing here is shared with oracle/.
 #pragma once
@@ -69,10 +69,9 @@ __device__ __forceinline__ bool key_less(uint64_t ka, uint32_t ia, uint64_t kb, 
 }
 
 // ---------------------------------------------------------------------------------------------- work lists
-// Per scheduler round: the fast kernel visits every replica and queues the ones it does not handle itself into
+// Per scheduler round: the streaming kernel visits every replica and queues the ones it does not handle itself into
 // list[cls * R + i], count[cls]; cls 0 = S (1 warp), 1 = M (4 warps), 2 = L (8 warps), 3 = overflow (a window that
-// outgrew its team during the round), 4 = windows of 65..128 requests for the second lean instance.
-// count[5] = replicas that have finished their trace (monotone).
+// outgrew its team during the round).  count[5] = replicas that have finished their trace (monotone).
 struct StepArgs {
   SimDev s;
   uint32_t* list; uint32_t* count;

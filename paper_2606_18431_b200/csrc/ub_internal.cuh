@@ -23,8 +23,11 @@ constexpr int64_t  kNever     = INT64_MAX;          // a_next when the trace is 
 constexpr uint32_t F_RESIDENT = 1u;        // KV on the device
 constexpr uint32_t F_SWAPPED  = 2u;        // KV in the host swap pool
 constexpr uint32_t F_EMITPREV = 4u;        // emitted a token in the previous executed iteration => t_last == clock
-constexpr uint32_t F_DIRTY    = 8u;        // hint: (class,key) may differ from the previous iteration's
-constexpr int      F_LOCK_SHIFT = 4;       // bits 4..31: lockbin + 1 (0 = no lock)
+constexpr uint32_t F_DIRTY    = 8u;        // (class,key) may differ from the previous iteration's => listed in dlist
+constexpr uint32_t F_ADMITNOW = 16u;       // admitted in the last executed iteration (read by the eviction pass only)
+constexpr uint32_t F_KLASS1   = 32u;       // was in class 1 (not MemGuard-locked) in the last executed iteration
+constexpr int      F_LOCK_SHIFT = 6;       // bits 6..31: lockbin + 1 (0 = no lock)
+constexpr uint32_t kDirtyMax  = 32;        // entries of a replica's dirty list; Hdr::n_dirty > kDirtyMax = overflow
 
 struct __align__(16) Rec0 { int64_t a; uint32_t P; uint32_t D; };
 struct __align__(16) Rec1 { uint32_t id; uint32_t d; uint32_t cached; uint32_t flags; };
@@ -39,7 +42,7 @@ struct __align__(16) Hdr {
   int64_t  iterations;
   uint32_t n_active, next, swap_used, peak_active;
   uint32_t n_completed, evict_recompute, evict_swap, swapins;
-  uint32_t done, pad0, pad1, pad2;
+  uint32_t done, todo, n_dirty, pad2;   // todo: iterations of this round still to do (hand-over between kernels)
 };
 static_assert(sizeof(Hdr) == 160, "Hdr is 160 bytes");
 
@@ -67,12 +70,14 @@ struct SimDev {                 // kernel argument (by value)
   int64_t* t_first; int64_t* t_last;      // [R][N]
   uint32_t* n_evict; uint32_t* n_evict_unf;
   uint32_t* hist;               // [R][kTbtBins]
+  uint16_t* dlist;              // [R][kDirtyMax] window positions of the re-keyed ("dirty") requests
+  uint2*    evbuf;              // [R][evcap] scratch: per-request events of one iteration that wait for t_end
+  uint32_t  evcap;              // min(M, Q)
 };
 
 // kernels (ub_step.cu, ub_aux.cu)
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, cudaStream_t st);
-void launch_fast(const struct StepArgs& A, cudaStream_t st);      // ub_fast.cu
-int  fast_configure();
+void launch_stream(const struct StepArgs& A, cudaStream_t st);    // ub_stream.cu
 size_t step_smem_bytes(uint32_t Q);
 int  step_configure(uint32_t Q);
 void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,

@@ -39,6 +39,7 @@ struct TeamScratch {            // per team, in shared memory
   unsigned long long bc64[8];
   unsigned long long acc64[6];  // rare-event accumulators
   uint32_t acc32[4];
+  uint32_t ndirty;             // next iteration's dirty-list length
 };
 
 template <int WARPS> struct Team {
@@ -238,7 +239,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
     }
     if (tid < 6) ts->acc64[tid] = 0ull;
     if (tid < 4) ts->acc32[tid] = 0u;
-    if (tid == 0) ts->bc[0] = 0xFFFFFFFFu;
+    if (tid == 0) { ts->bc[0] = 0xFFFFFFFFu; ts->ndirty = 0u; }
     tm.sync();
 
     // ---------------- a2: order.  The stored order is last iteration's priority order (MemGuard keeps keys
@@ -595,6 +596,10 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         if (keep) {
           *reinterpret_cast<int4*>(gE0 + np) = *reinterpret_cast<const int4*>(&r0[c]);
           *reinterpret_cast<int4*>(gE1 + np) = *reinterpret_cast<const int4*>(&r1[c]);
+          if (r1[c].flags & F_DIRTY) {                       // the streaming kernel's dirty list (ub_stream.cu)
+            const uint32_t slot = atomicAdd(&ts->ndirty, 1u);
+            if (slot < kDirtyMax) s.dlist[(size_t)r * kDirtyMax + slot] = (uint16_t)np;
+          }
         }
         n_new += tot;
       }
@@ -602,6 +607,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
 
     // ---------------- header words (thread i of warp 0 owns word i)
     if (tid == 0 && tot2[1]) atomicAdd(&g_hist[tbt_bin(cost)], tot2[1]);
+    tm.sync();                                   // ts->ndirty complete
     {
       const uint32_t evs_lo = ev2[0] + ts->acc32[2], evs_hi = ev2[1] + ts->acc32[3];
       const uint32_t n_done = ts->acc32[0];
@@ -624,6 +630,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
           case 14: { uint32_t pk = (uint32_t)(hv >> 32); if (n > pk) pk = n; hv = (uint64_t)swap_used | ((uint64_t)pk << 32); } break;
           case 15: hv += (uint64_t)n_done + ((uint64_t)ev_nrc << 32); break;
           case 16: hv += (uint64_t)ev_nsw + ((uint64_t)swin_cnt << 32); break;
+          case 18: { const uint32_t q = ts->ndirty; hv = (hv & 0xFFFFFFFF00000000ull) | (q > kDirtyMax ? kDirtyMax + 1u : q); } break;
           default: break;
         }
       }
@@ -684,21 +691,20 @@ int step_configure(uint32_t) {
   if (e == cudaSuccess)
     e = cudaFuncSetAttribute(k_step<1, kES, kTeamsS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(kTeamsS * TeamSmem<1, kES>::BYTES));
-  if (e == cudaSuccess) return fast_configure();
   return (int)e;
 }
 
-// One scheduler round (`iters` iterations of every live replica): the fast kernel visits every replica and queues
-// what it does not handle (large windows, evictions, re-sorts) for the team kernels: L list, M list, S list, then
-// the overflow list.
+// One scheduler round (`iters` iterations of every live replica): the streaming kernel (ub_stream.cu) visits every
+// replica and queues what it does not handle (SRPT / LAS keys, test-only modes, re-key bursts) for the team kernels:
+// L list, M list, S list, then the overflow list.
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, cudaStream_t st) {
   StepArgs A;
   A.s = s; A.list = list; A.count = count; A.iters = iters;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
-  cudaMemsetAsync(count, 0, 5 * sizeof(uint32_t), st);                          // this round's lists start empty
-  launch_fast(A, st);
+  cudaMemsetAsync(count, 0, 4 * sizeof(uint32_t), st);                          // this round's lists start empty
+  launch_stream(A, st);
   const uint32_t R = s.R;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;
   const uint32_t nS = (R + kTeamsS - 1) / kTeamsS, gS = nS < 148u * 10 ? nS : 148u * 10;

@@ -1,0 +1,550 @@
+// ub_stream.cu -- the streaming scheduling-step kernel of libuniboost.so (sm_100a): ONE WARP advances one replica by
+// one (or `iters`) scheduler iterations of Algorithm 1 under the model rules M1..M12 of DESIGN.md
+// Sec. 3, for a window of any size up to the queue cap.
+//
+// The replica's active window is kept in HBM in the priority order of the last iteration.  MemGuard keeps keys
+// piecewise constant: between two iterations only the few requests whose (residency, bin, class)
+// changed -- listed by the previous iteration in the replica's dirty list -- and the new arrivals can change place.
+// One iteration is ONE pass over the window, 32 requests per chunk, one 16-byte record of each array per lane, the
+// next chunk in flight while the current one is processed:
+//   a0 ingest / idle jump (M6)    arrivals are read from the packed trace
+//   a1 score (M3-M5)              boost table held in registers (lane b holds LUT[b]), looked up by shuffle
+//   a2 order                      the dirty requests and the arrivals (<= 32 together) are scored, ranked against each
+//                                 other in-warp and merged into the stream of the other, still sorted, requests
+//   a3 admit (M7)                 the walk is a carried state machine over the chunks: two warp scans per chunk
+//                                 (tokens, KV blocks), a ballot for the first misfit, "residents only" behind a
+//                                 blocked newcomer, nothing once the walk has stopped
+//   a5 advance (M9-M10, M12)      applied in the same pass, records rewritten in place (E1 when it changed, E0 only
+//                                 where the order shifts); what needs the iteration's end time (first token, gap
+//                                 after a stall, completion) is queued and applied when the cost is known
+//   a4 victim select (M8)         if the stalled residents no longer fit: one backward pass over the window tail
+// Integers only.  Not handled here, decided before any write and queued for the team kernels of ub_step.cu: the
+// SRPT / LAS keys (they drift every token), the test-only signal / quantiser modes, a block size that is not a power
+// of two, more than 32 dirty requests + arrivals in one iteration.
+#include "ub_device.cuh"
+
+namespace ub {
+
+constexpr int kSWarps = 4;                 // warps per CTA, each streams its own replicas
+constexpr uint32_t kFull = 0xffffffffu;
+
+// inclusive warp scan, one SHFL + one predicated add per step (the shuffle's own "source lane in range" predicate)
+__device__ __forceinline__ uint32_t scan32(uint32_t v) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    asm volatile("{ .reg .u32 t; .reg .pred p; shfl.sync.up.b32 t|p, %0, %1, 0x0, 0xffffffff; @p add.u32 %0, %0, t; }"
+                 : "+r"(v) : "r"(o));
+  }
+  return v;
+}
+
+struct __align__(16) SideStash {           // per warp: the dirty requests + arrivals of one iteration, in key order
+  uint4 r0[32];
+  uint4 r1[32];
+  uint4 kb[32];                            // {key lo, key hi, bin, -}
+};
+
+// a1 (M3-M5): sig = P + d; bin = Eq. 8 exponent; pi = a - b_gamma(w_hat) - delta if
+// resident (Eq. 7); key = class<<63 | (pi + 2^62); class 0 = MemGuard-locked resident.  All 32 lanes must call it.
+__device__ __forceinline__ void score(const Rec0& q0, const Rec1& q1, uint32_t k, int64_t lutv, int64_t delta,
+                                      bool guard, uint64_t& key, uint32_t& bin) {
+  const uint32_t sig = q0.P + q1.d;
+  const uint32_t sg = sig > k ? sig : k;
+  uint32_t b = (uint32_t)(__clz(k) - __clz(sg));
+  b -= ((k << b) > sg) ? 1u : 0u;
+  const uint32_t lo = __shfl_sync(kFull, (uint32_t)lutv, (int)b);
+  const uint32_t hi = __shfl_sync(kFull, (uint32_t)((uint64_t)lutv >> 32), (int)b);
+  const bool res = (q1.flags & F_RESIDENT) != 0;
+  const int64_t kv = q0.a - (int64_t)(((uint64_t)hi << 32) | lo) - (res ? delta : 0ll);
+  const bool locked = guard && res && (q1.flags >> F_LOCK_SHIFT) == b + 1u;
+  key = (uint64_t)(kv + kKeyBias) | (locked ? 0ull : (1ull << 63));
+  bin = b;
+}
+
+__global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
+  __shared__ SideStash stash[kSWarps];
+  const SimDev& s = A.s;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const uint32_t ltmask = (1u << lane) - 1u;
+  SideStash& X = stash[wib];
+  const uint32_t B = s.B, M = s.M, cc = s.c, Tb = s.T, Q = s.Q, k = s.k;
+  const uint32_t blk_m1 = s.blk - 1u, blk_sh = s.blk_shift;
+  const uint32_t nwarps = gridDim.x * kSWarps;
+
+  for (uint32_t r = blockIdx.x * kSWarps + wib; r < s.R; r += nwarps) {
+    // ---- everything whose address depends on r only is requested at once: header words (Hdr, ub_internal.cuh;
+    // uniform loads), parameters, the first chunk of the window and the dirty list (speculatively)
+    unsigned long long* h64 = reinterpret_cast<unsigned long long*>(s.hdr + r);
+    Rec0* gE0 = s.E0 + (size_t)r * Q;
+    Rec1* gE1 = s.E1 + (size_t)r * Q;
+    const unsigned long long w13 = __ldcg(h64 + 13);
+    int64_t a_next = (int64_t)__ldcg(h64 + 2);
+    int64_t t = (int64_t)__ldcg(h64 + 0);
+    uint64_t H = __ldcg(h64 + 1);
+    const unsigned long long w14 = __ldcg(h64 + 14);
+    uint32_t nd = (uint32_t)__ldcg(h64 + 18);                         // entries of the dirty list
+    const RepPar par = s.par[r];
+    int4 p0 = make_int4(0, 0, 0, 0), p1 = make_int4(0, 0, 0, 0);
+    if ((uint32_t)lane < Q) {
+      p0 = __ldcg(reinterpret_cast<const int4*>(gE0 + lane));
+      p1 = __ldcg(reinterpret_cast<const int4*>(gE1 + lane));
+    }
+    uint32_t pdl = __ldcg(s.dlist + (size_t)r * kDirtyMax + lane);
+    uint32_t n = (uint32_t)w13, next = (uint32_t)(w13 >> 32);
+    if (n == 0 && a_next == kNever) continue;                         // finished its trace
+    uint32_t swap_used = (uint32_t)w14, peak = (uint32_t)(w14 >> 32);
+    const uint32_t iters = A.iters;
+
+    const Rec0* TR = s.TR + (size_t)par.trace_id * s.N;
+    uint16_t* gdl = s.dlist + (size_t)r * kDirtyMax;
+    const bool isboost = par.policy == 2;
+    const int64_t delta = par.delta;
+    const bool guard = par.guard != 0;
+
+    // the streaming path covers the arrival-keyed policies with the paper's signal and quantiser
+    bool slow = !(par.policy == 0 || par.policy == 2) || par.signal_mode != 0 || par.quant_mode != 0 || blk_sh >= 32u;
+    // boost table in registers: lane b holds LUT[b] (Eq. 2 in fixed point, built on the host, M4); FCFS: all 0
+    int64_t lutv = 0;
+    if (isboost && !slow) lutv = __ldg(s.lut + par.lut_off + lane);   // geometric tables have 64 entries, bins < 32
+    uint32_t it = 0;
+    uint32_t wsize = n;
+
+    for (; !slow && it < iters; it++) {
+      // ---------------- a0: idle jump + ingest (M6)
+      if (n == 0) {
+        if (a_next == kNever) break;
+        if (a_next > t) t = a_next;
+      }
+      uint32_t cnt = 0, nreq = 0;
+      if (a_next <= t && n < Q) {                                     // a_next != kNever => next < nreq
+        nreq = __ldg(s.n_req + par.trace_id);
+        const uint32_t avail = (Q - n) < (nreq - next) ? (Q - n) : (nreq - next);
+        const bool take = (uint32_t)lane < avail && __ldg(&TR[next + lane].a) <= t;   // arrivals sorted => a prefix
+        cnt = __popc(__ballot_sync(kFull, take));
+        if (cnt == 32u && avail > 32u) cnt = 64u;                     // maybe more: not for this kernel
+      }
+      wsize = n + cnt;
+      if (nd + cnt > kDirtyMax) { slow = true; break; }               // (nd > kDirtyMax marks a list that overflowed)
+      const uint32_t n_old = n, m = nd + cnt;
+      n += cnt;
+
+      // ---------------- a2 (first half): the requests that may change place -- dirty ones and arrivals -- are taken
+      // out of the stream, scored, ranked among themselves by (class, key, id) and parked in shared memory
+      uint32_t spos = 0xFFFFFFFFu;                                    // window position a dirty request is taken from
+      if (m) {
+        int4 v0 = make_int4(0, 0, 0, 0), v1 = make_int4(0, 0, 0, 0);
+        if ((uint32_t)lane < nd) {
+          spos = pdl;
+          v0 = __ldcg(reinterpret_cast<const int4*>(gE0 + spos));
+          v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + spos));
+        } else if ((uint32_t)lane < m) {
+          const uint32_t i = next + ((uint32_t)lane - nd);
+          v0 = __ldg(reinterpret_cast<const int4*>(TR + i));
+          v1 = make_int4((int)i, 0, 0, 0);
+        }
+        if (cnt) {
+          next += cnt;
+          a_next = (next < nreq) ? __ldg(&TR[next].a) : kNever;
+        }
+        const Rec0 q0 = *reinterpret_cast<const Rec0*>(&v0);
+        const Rec1 q1 = *reinterpret_cast<const Rec1*>(&v1);
+        uint64_t sk; uint32_t sb;
+        score(q0, q1, k, lutv, delta, guard, sk, sb);
+        uint32_t rank = 0;
+        if (m > 1u) {
+          for (uint32_t j = 0; j < m; j++) {
+            const uint64_t kj = __shfl_sync(kFull, sk, (int)j);
+            const uint32_t ij = __shfl_sync(kFull, q1.id, (int)j);
+            rank += key_less(kj, ij, sk, q1.id) ? 1u : 0u;
+          }
+        }
+        if ((uint32_t)lane < m) {
+          X.r0[rank] = *reinterpret_cast<const uint4*>(&v0);
+          X.r1[rank] = *reinterpret_cast<const uint4*>(&v1);
+          X.kb[rank] = make_uint4((uint32_t)sk, (uint32_t)(sk >> 32), sb, 0u);
+        }
+        __syncwarp();
+      }
+
+      // ---------------- the pass.  Walk state (M7), warp-uniform: mode 0 = everybody walks, 1 = residents only (a
+      // newcomer was blocked on KV), 2 = stopped; carryW / carryC = tokens / KV blocks claimed so far; crank = rank of
+      // the next request in the merged order; carryN = requests admitted so far (mode 1).
+      uint32_t mode = 0, carryW = 0, carryC = 0, carryN = 0, crank = 0;
+      uint32_t pf = 0, dec = 0, kres = 0, evl = 0, evu = 0, emit = 0, same = 0, swb = 0, swc = 0;   // per-lane sums
+      uint32_t outpos = 0, nev = 0, ndnew = 0, n_done = 0;
+      uint32_t dptr = 0;                                              // next parked request to merge
+
+      // one segment of the merged order: the lanes of `mask`, in lane order
+      auto process = [&](const Rec0& w0, const Rec1& w1, const uint64_t key, const uint32_t bin, const uint32_t mask,
+                         const uint32_t stpos) {
+        const bool valid = (mask >> lane) & 1u;
+        const uint32_t of = w1.flags;
+        const bool res = valid && (of & F_RESIDENT) != 0;
+        const uint32_t rem = w0.P + w1.d - w1.cached;
+        uint32_t want = 0;
+        // ---- a3: admission walk as prefix scans (M7; Algorithm 1 "while |B| < M ... U + dU <= B")
+        //   W = incl. scan of min(c, rem);  tok_before = min(T, W - w);  want = min(T, W) - tok_before;
+        //   foot = ceil((cached + want)/blk);  Cf = incl. scan of foot;  ok = rank < M & tok_before < T & Cf <= B.
+        // ok is monotone along the walk: the admitted set is the prefix in front of the first misfit.  If that one is
+        // a non-resident that failed on KV only ("newblocked"), the walk continues over the residents behind it.
+        if (mode < 2u) {
+          const uint32_t resm = __ballot_sync(kFull, res);
+          uint32_t pm = mode == 0u ? mask : resm;
+          uint32_t from = 0;                                          // lanes below `from` are settled
+          while (pm) {                                                // at most two rounds per segment
+            const bool part = (pm >> lane) & 1u;
+            const uint32_t w = part ? (rem < cc ? rem : cc) : 0u;
+            const uint32_t W = carryW + scan32(w);
+            const uint32_t tok_before = (W - w) < Tb ? (W - w) : Tb;
+            const uint32_t tok_after = W < Tb ? W : Tb;
+            const uint32_t wnt = tok_after - tok_before;
+            const uint32_t foot = part ? (w1.cached + wnt + blk_m1) >> blk_sh : 0u;
+            const uint32_t Cf = carryC + scan32(foot);
+            const uint32_t cb = (mode == 0u ? crank : carryN) + __popc(pm & ltmask);
+            const bool ok = part && cb < M && tok_before < Tb && Cf <= B;
+            if (ok) want = wnt;
+            const uint32_t fm = __ballot_sync(kFull, part && !ok);
+            if (!fm) {
+              carryW = __shfl_sync(kFull, W, 31);
+              carryC = __shfl_sync(kFull, Cf, 31);
+              carryN += __popc(pm);
+              break;
+            }
+            const int fl = __ffs(fm) - 1;                             // the first request that did not fit
+            const uint32_t fC = __shfl_sync(kFull, Cf - foot, fl);
+            const uint32_t ftok = __shfl_sync(kFull, tok_before, fl);
+            const uint32_t fcb = __shfl_sync(kFull, cb, fl);
+            carryC = fC; carryW = ftok; carryN = fcb;
+            if (mode == 0u && fcb < M && ftok < Tb && !((resm >> fl) & 1u)) {
+              mode = 1u;                                              // newblocked: residents behind it continue
+              from = (uint32_t)fl + 1u;
+              pm = from < 32u ? (resm & (kFull << from)) : 0u;
+            } else {
+              mode = 2u;
+              pm = 0u;
+            }
+          }
+          (void)from;
+        }
+        crank += __popc(mask);
+
+        // ---- batch totals (M9) and events (M12)
+        const bool adm = want != 0u;
+        const bool isdec = adm && w1.d >= 1u && rem == 1u;            // decode sequence vs prefill tokens
+        dec += isdec ? 1u : 0u;
+        pf += isdec ? 0u : want;
+        {
+          const uint32_t m32 = ((w1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu);
+          const uint64_t h = (uint64_t)m32 * (uint64_t)(2u * want + 1u);
+          evl += adm ? (uint32_t)h : 0u;
+          evu += adm ? (uint32_t)(h >> 32) : 0u;
+        }
+        const bool swp = adm && (of & F_SWAPPED);
+        if (__any_sync(kFull, swp)) {                                 // swap-in on admission (rare)
+          if (swp) {
+            const uint32_t blocks = (w1.cached + blk_m1) >> blk_sh;
+            swb += blocks; swc++;
+            ev_add(evl, evu, EV_SWAPIN, w1.id, blocks);
+          }
+        }
+        kres += (res && !adm) ? (w1.cached + blk_m1) >> blk_sh : 0u;  // stalled residents keep their blocks (M8)
+
+        // ---- a5: apply (M10)
+        const uint32_t d_old = w1.d;
+        const uint32_t sig = w0.P + d_old;
+        const uint32_t cached2 = w1.cached + want;
+        const bool emitted = adm && cached2 == sig;                   // KV caught up => one token out (M2)
+        const bool ep_old = (of & F_EMITPREV) != 0;
+        const uint32_t d2 = d_old + (emitted ? 1u : 0u);
+        emit += emitted ? 1u : 0u;
+        same += (emitted && d_old != 0u && ep_old) ? 1u : 0u;         // gap == this iteration's cost
+        const bool gone = emitted && d2 == w0.D;                      // complete: KV freed at once
+        uint32_t nf = of & (F_RESIDENT | F_SWAPPED);
+        if (adm) nf = F_RESIDENT | F_ADMITNOW;
+        if (emitted) nf |= F_EMITPREV;
+        // re-lock at this iteration's bin (M10, G6); a request is dirty for the next iteration's ordering when
+        // (resident, bin, class) -- the inputs of its key -- change
+        const uint32_t b2 = bin + ((emitted && sig + 1u == (k << (bin + 1u))) ? 1u : 0u);
+        const bool res2 = (nf & F_RESIDENT) != 0;
+        const uint32_t klass = (uint32_t)(key >> 63);
+        const uint32_t klass2 = (guard && res2 && b2 == bin) ? 0u : 1u;
+        const bool dirty = (((nf ^ of) & F_RESIDENT) != 0) || (isboost && b2 != bin) || (klass2 != klass);
+        if (res2) nf |= (bin + 1u) << F_LOCK_SHIFT;
+        if (klass) nf |= F_KLASS1;
+        if (dirty) nf |= F_DIRTY;
+        const uint32_t gonem = __ballot_sync(kFull, gone);
+        // everything that touches the per-request outputs is rare: first token, a gap after a stall, completion,
+        // the end of an emission streak (t_last is implicit while a request emits every iteration)
+        const bool defer = emitted && (d_old == 0u || !ep_old || gone);
+        const bool ends = valid && !emitted && ep_old;
+        if (__any_sync(kFull, defer || ends)) {
+          if (ends) s.t_last[(size_t)r * s.N + w1.id] = t;                               // persist t_last when the streak ends
+          const uint32_t em = __ballot_sync(kFull, defer);
+          if (defer)
+            s.evbuf[(size_t)r * s.evcap + nev + __popc(em & ltmask)] =
+                make_uint2(w1.id, (d_old == 0u ? 1u : 0u) | ((d_old != 0u && !ep_old) ? 2u : 0u) | (gone ? 4u : 0u));
+          nev += __popc(em);
+        }
+
+        // ---- write back in priority order, dropping completed requests; untouched records stay put
+        const uint32_t keepm = mask & ~gonem;
+        const bool keep = (keepm >> lane) & 1u;
+        const uint32_t np = outpos + __popc(keepm & ltmask);
+        const bool moved = np != stpos;
+        if (keep && moved) __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&w0));
+        if (keep && (moved || adm || nf != of))
+          __stcg(reinterpret_cast<int4*>(gE1 + np), make_int4((int)w1.id, (int)d2, (int)cached2, (int)nf));
+        const uint32_t dm = __ballot_sync(kFull, keep && dirty);
+        if (dm) {                                                     // next iteration's dirty list
+          const uint32_t slot = ndnew + __popc(dm & ltmask);
+          if (keep && dirty && slot < kDirtyMax) gdl[slot] = (uint16_t)np;
+          ndnew += __popc(dm);
+        }
+        outpos += __popc(keepm);
+        n_done += __popc(gonem);
+      };
+
+      const uint32_t nch = (n_old + 31u) >> 5;
+      int4 nx0 = make_int4(0, 0, 0, 0), nx1 = make_int4(0, 0, 0, 0);
+      if ((uint32_t)lane < n_old) { nx0 = p0; nx1 = p1; }
+      for (uint32_t c = 0; c <= nch; c++) {
+        if (c == nch && dptr >= m) break;                             // (chunk nch is empty: the parked tail)
+        const int4 c0 = nx0, c1 = nx1;
+        {
+          const uint32_t pn = (c + 1u) * 32u + (uint32_t)lane;
+          nx0 = make_int4(0, 0, 0, 0); nx1 = make_int4(0, 0, 0, 0);
+          if (pn < n_old) {
+            nx0 = __ldcg(reinterpret_cast<const int4*>(gE0 + pn));
+            nx1 = __ldcg(reinterpret_cast<const int4*>(gE1 + pn));
+          }
+        }
+        const Rec0 r0 = *reinterpret_cast<const Rec0*>(&c0);
+        const Rec1 r1 = *reinterpret_cast<const Rec1*>(&c1);
+        const uint32_t left = c < nch ? n_old - c * 32u : 0u;
+        uint32_t cv = left >= 32u ? kFull : ((1u << left) - 1u);      // requests of this chunk still in the stream
+        uint64_t key; uint32_t bin;
+        score(r0, r1, k, lutv, delta, guard, key, bin);
+        if (m) {
+          if (nd)
+            cv &= ~__reduce_or_sync(kFull, ((uint32_t)lane < nd && (spos >> 5) == c) ? (1u << (spos & 31u)) : 0u);
+          // writes of this chunk may reach into the next one when parked requests are merged in front of it: the
+          // next chunk must have arrived in registers before anything is stored
+          uint32_t dummy;
+          asm volatile("{ .reg .pred p; setp.eq.u32 p, %1, %2; vote.sync.ballot.b32 %0, p, 0xffffffff; }"
+                       : "=r"(dummy) : "r"(nx0.x), "r"(nx1.w) : "memory");
+          (void)dummy;
+          __syncwarp();
+        }
+        uint32_t lo = 0;
+        for (;;) {
+          uint32_t fl = 32;
+          if (dptr < m) {                                             // clean requests that sort behind the next parked one
+            const uint4 dk = X.kb[dptr];
+            const uint32_t di = X.r1[dptr].x;
+            const uint32_t after = __ballot_sync(kFull, ((cv >> lane) & 1u) && (uint32_t)lane >= lo &&
+                                                 key_less((uint64_t)dk.x | ((uint64_t)dk.y << 32), di, key, r1.id));
+            if (after) fl = (uint32_t)__ffs(after) - 1u;
+          }
+          const uint32_t seg = cv & (fl < 32u ? ((1u << fl) - 1u) : kFull) & (lo < 32u ? (kFull << lo) : 0u);
+          if (seg) process(r0, r1, key, bin, seg, c * 32u + (uint32_t)lane);
+          lo = fl;
+          if ((fl == 32u && c < nch) || dptr >= m) break;
+          uint32_t j = m - dptr;                                      // parked requests in front of clean lane fl
+          if (fl < 32u) {
+            const uint64_t ck = __shfl_sync(kFull, key, (int)fl);
+            const uint32_t ci = __shfl_sync(kFull, r1.id, (int)fl);
+            const uint4 kb = X.kb[lane];
+            j = __popc(__ballot_sync(kFull, (uint32_t)lane >= dptr && (uint32_t)lane < m &&
+                                     key_less((uint64_t)kb.x | ((uint64_t)kb.y << 32), X.r1[lane].x, ck, ci)));
+          }
+          {
+            const uint32_t src = dptr + (uint32_t)lane < 32u ? dptr + (uint32_t)lane : 31u;
+            const uint4 a0 = X.r0[src], a1 = X.r1[src], ak = X.kb[src];
+            process(*reinterpret_cast<const Rec0*>(&a0), *reinterpret_cast<const Rec1*>(&a1),
+                    (uint64_t)ak.x | ((uint64_t)ak.y << 32), ak.z, j < 32u ? ((1u << j) - 1u) : kFull, 0xFFFFFFFFu);
+          }
+          dptr += j;
+        }
+      }
+      __syncwarp();
+
+      // ---------------- batch totals, victim select, cost
+      pf = __reduce_add_sync(kFull, pf);
+      const uint32_t de = __reduce_add_sync(kFull, dec | (emit << 16));
+      dec = de & 0xFFFFu; emit = de >> 16;
+      same = __reduce_add_sync(kFull, same);
+      kres = __reduce_add_sync(kFull, kres);
+      uint32_t swin_blocks = 0, swin_cnt = 0;
+      if (__any_sync(kFull, swc != 0u)) {
+        swin_blocks = __reduce_add_sync(kFull, swb);
+        swin_cnt = __reduce_add_sync(kFull, swc);
+        swap_used -= swin_blocks;
+      }
+      const uint32_t C = carryC;
+      const uint32_t n_new = outpos;
+      uint32_t swout_blocks = 0, ev_nsw = 0, ev_nrc = 0;
+      uint64_t ev_lost = 0;
+      if (kres > B - C) {
+        // ---- a4 (M8; SELECTVICTIM / SWAPOUT): the stalled residents (resident, not admitted) no
+        // longer fit behind the claims.  Victims = the suffix of them, in priority order, whose inclusive prefix sum
+        // of blocks exceeds B - C; lowest priority first, the swap pool being a sequential resource.
+        const uint32_t thr = B - C;
+        uint32_t behind = 0;                                          // blocks of stalled residents behind this chunk
+        for (int c = (int)((n_new - 1u) >> 5); c >= 0; c--) {
+          const uint32_t pos = (uint32_t)c * 32u + (uint32_t)lane;
+          int4 v1 = make_int4(0, 0, 0, 0);
+          if (pos < n_new) v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + pos));
+          Rec1 q = *reinterpret_cast<Rec1*>(&v1);
+          const bool st = pos < n_new && (q.flags & F_RESIDENT) && !(q.flags & F_ADMITNOW);
+          const uint32_t v = st ? (q.cached + blk_m1) >> blk_sh : 0u;
+          const uint32_t inc = scan32(v);
+          const uint32_t tot = __shfl_sync(kFull, inc, 31);
+          const uint32_t prefix = kres - behind - (tot - inc);        // blocks of stalled residents up to and with me
+          const bool victim = st && prefix > thr;
+          uint32_t vm = __ballot_sync(kFull, victim);
+          const uint32_t allvm = vm;
+          const uint32_t of = q.flags;
+          while (vm) {
+            const int l = 31 - __clz((int)vm); vm &= ~(1u << l);
+            const uint32_t cached_l = __shfl_sync(kFull, q.cached, l);
+            const uint32_t id_l = __shfl_sync(kFull, q.id, l);
+            const uint32_t resb = (cached_l + blk_m1) >> blk_sh;
+            bool do_swap = false;
+            if (s.preempt_mode == 1) do_swap = (swap_used + resb <= s.swap_pool);
+            else if (s.preempt_mode == 2)
+              do_swap = (swap_used + resb <= s.swap_pool) &&
+                        (2ll * resb * (int64_t)s.swap_ns < 1000ll * s.c_pf * (int64_t)cached_l);
+            if (do_swap) {
+              swap_used += resb; swout_blocks += resb; ev_nsw++;
+              if (lane == 0) ev_add(evl, evu, EV_EVICT_SWAP, id_l, resb);
+              if (lane == l) q.flags = F_SWAPPED | F_DIRTY;
+            } else {
+              ev_lost += cached_l; ev_nrc++;
+              if (lane == 0) ev_add(evl, evu, EV_EVICT_RECOMPUTE, id_l, cached_l);
+              if (lane == l) { q.cached = 0; q.flags = F_DIRTY; }
+            }
+          }
+          if (victim) {
+            uint32_t* g_ne = s.n_evict + (size_t)r * s.N;
+            g_ne[q.id] = __ldcg(g_ne + q.id) + 1u;
+            if (of & F_KLASS1) {                                      // victim was not MemGuard-locked
+              uint32_t* g_neu = s.n_evict_unf + (size_t)r * s.N;
+              g_neu[q.id] = __ldcg(g_neu + q.id) + 1u;
+            }
+            __stcg(reinterpret_cast<int4*>(gE1 + pos), *reinterpret_cast<const int4*>(&q));
+          }
+          const uint32_t dm = __ballot_sync(kFull, victim && !(of & F_DIRTY));      // residency changed => dirty
+          if (dm) {
+            const uint32_t slot = ndnew + __popc(dm & ltmask);
+            if (victim && !(of & F_DIRTY) && slot < kDirtyMax) gdl[slot] = (uint16_t)pos;
+            ndnew += __popc(dm);
+          }
+          behind += tot;
+          if (__ballot_sync(kFull, st) != allvm) break;               // a stalled resident that stays: so do all before it
+        }
+      }
+      const int64_t cost = s.c0 + s.c_pf * (int64_t)pf + s.c_dec * (int64_t)dec +
+                           (int64_t)(((uint64_t)(swin_blocks + swout_blocks) * s.swap_ns + 500u) / 1000u);
+      const int64_t t_end = t + cost;
+
+      // ---------------- the queued per-request events, now that t_end is known (M10, M11)
+      if (nev) {
+        const uint2* gev = s.evbuf + (size_t)r * s.evcap;
+        int64_t* g_tfirst = s.t_first + (size_t)r * s.N;
+        int64_t* g_tlast = s.t_last + (size_t)r * s.N;
+        for (uint32_t e0 = 0; e0 < nev; e0 += 32u) {
+          const uint32_t e = e0 + (uint32_t)lane;
+          if (e < nev) {
+            const uint2 ev = __ldcg(gev + e);
+            const uint32_t id = ev.x;
+            if (ev.y & 1u) {
+              g_tfirst[id] = t_end;
+              ev_add(evl, evu, EV_EMIT_FIRST, id, 0u);
+            }
+            if (ev.y & 2u) {
+              const int64_t tl = __ldcg(g_tlast + id);
+              atomicAdd(s.hist + (size_t)r * kTbtBins + tbt_bin(t_end - tl), 1u);
+            }
+            if (ev.y & 4u) {
+              g_tlast[id] = t_end;
+              const int64_t tf = (ev.y & 1u) ? t_end : __ldcg(g_tfirst + id);
+              const int4 tv = __ldg(reinterpret_cast<const int4*>(TR + id));
+              const Rec0 q0 = *reinterpret_cast<const Rec0*>(&tv);
+              atomicAdd(h64 + 8, (unsigned long long)(tf - q0.a));
+              atomicAdd(h64 + 9, (unsigned long long)(t_end - q0.a));
+              atomicAdd(h64 + 10, (unsigned long long)(t_end - tf));
+              atomicAdd(h64 + 11, (unsigned long long)(q0.D - 1u));
+              ev_add(evl, evu, EV_COMPLETE, id, 0u);
+              uint32_t* g_ne = s.n_evict + (size_t)r * s.N;
+              g_ne[id] = __ldcg(g_ne + id) | 0x80000000u;             // completion marker read by the stats kernel
+            }
+          }
+        }
+      }
+      evl = __reduce_add_sync(kFull, evl);
+      evu = __reduce_add_sync(kFull, evu);
+
+      // ---------------- header: clock, digest (M12), cursors; counters by RED (no read needed)
+      H = digest_fold(H, evl, evu, t_end);
+      if (ndnew > kDirtyMax) ndnew = kDirtyMax + 1u;
+      if (lane == 0) {
+        if (same) atomicAdd(s.hist + (size_t)r * kTbtBins + tbt_bin(cost), same);
+        __stcg(h64 + 0, (unsigned long long)t_end);
+        __stcg(h64 + 1, (unsigned long long)H);
+        if (cnt) __stcg(h64 + 2, (unsigned long long)a_next);
+        __stcg(h64 + 13, (unsigned long long)n_new | ((unsigned long long)next << 32));
+        if (n > peak || swin_blocks || swout_blocks)
+          __stcg(h64 + 14, (unsigned long long)swap_used | ((unsigned long long)(n > peak ? n : peak) << 32));
+        if (ndnew != nd) __stcg(reinterpret_cast<uint32_t*>(h64 + 18), ndnew);
+        atomicAdd(h64 + 3, (unsigned long long)n);                    // request-steps
+        atomicAdd(h64 + 4, (unsigned long long)emit);
+        if (pf) atomicAdd(h64 + 5, (unsigned long long)pf);
+        atomicAdd(h64 + 6, (unsigned long long)dec);
+        if (ev_lost) atomicAdd(h64 + 7, (unsigned long long)ev_lost);
+        atomicAdd(h64 + 12, 1ull);                                    // iterations
+        if (n_done | ev_nrc) atomicAdd(h64 + 15, (unsigned long long)n_done | ((unsigned long long)ev_nrc << 32));
+        if (ev_nsw | swin_cnt) atomicAdd(h64 + 16, (unsigned long long)ev_nsw | ((unsigned long long)swin_cnt << 32));
+      }
+      if (n > peak) peak = n;
+      t = t_end; n = n_new; wsize = n_new; nd = ndnew;
+      if (n == 0 && a_next == kNever) {                               // finished its trace in this call
+        if (lane == 0) atomicAdd(A.count + 5, 1u);
+        it++;
+        break;
+      }
+      __syncwarp();                                                   // window stores before the next iteration's loads
+      if (it + 1u < iters) {
+        if ((uint32_t)lane < Q) {
+          p0 = __ldcg(reinterpret_cast<const int4*>(gE0 + lane));
+          p1 = __ldcg(reinterpret_cast<const int4*>(gE1 + lane));
+        }
+        pdl = __ldcg(gdl + lane);
+      }
+    }
+
+    // ---------------- not handled here: queue the replica for the team kernels of this round
+    if (slow && lane == 0) {
+      if (it > 0) reinterpret_cast<uint32_t*>(h64 + 17)[1] = iters - it;       // iterations still to do
+      push_list(A, wsize <= A.thrS ? 0u : (wsize <= A.thrM ? 1u : 2u), r);
+    }
+  }
+}
+
+// persistent grid: every warp strides over the replicas
+void launch_stream(const StepArgs& A, cudaStream_t st) {
+  static int ctas_per_sm = 0;
+  if (!ctas_per_sm) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream, 32 * kSWarps, 0) != cudaSuccess ||
+        ctas_per_sm < 1)
+      ctas_per_sm = 4;
+  }
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const uint32_t need = (A.s.R + kSWarps - 1) / kSWarps;
+  uint32_t grid = (uint32_t)(sms * ctas_per_sm);
+  if (grid > need) grid = need;
+  k_stream<<<grid, 32 * kSWarps, 0, st>>>(A);
+}
+
+}  // namespace ub
