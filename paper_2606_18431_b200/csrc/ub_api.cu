@@ -84,7 +84,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
   s->last_ms = 0.f; s->last_launches = 0;
   const size_t R = c->n_replicas, Q = c->queue_cap, N = c->max_requests, NT = c->n_traces;
   int rc = UB_OK;
-  if ((rc = dmalloc(&s->d_E0, R * Q)) || (rc = dmalloc(&s->d_E1, R * Q)) || (rc = dmalloc(&s->d_hdr, R)) ||
+  if ((rc = dmalloc(&s->d_E0, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_E1, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_hdr, R)) ||
       (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
@@ -256,6 +256,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
     RepPar& p = par[r];
     p.delta = q.hysteresis_us; p.trace_id = q.trace_id; p.lut_off = off; p.lut_nb = nb;
     p.policy = q.policy; p.guard = q.guard; p.signal_mode = q.signal_mode; p.quant_mode = q.quant_mode;
+    p.pad[0] = p.pad[1] = 0;
   }
   cudaFree(s->d_lut); s->d_lut = nullptr;
   int rc = dmalloc(&s->d_lut, s->h_lut.size()); if (rc) return rc;

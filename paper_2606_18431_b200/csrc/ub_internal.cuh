@@ -46,13 +46,15 @@ struct __align__(16) Hdr {
 };
 static_assert(sizeof(Hdr) == 160, "Hdr is 160 bytes");
 
-struct __align__(8) RepPar {    // per-replica parameters, read-only on the device
+struct __align__(16) RepPar {   // per-replica parameters, read-only on the device (32 bytes: two cp.async pieces)
   int64_t  delta;               // hysteresis_us
   uint32_t trace_id;
   uint32_t lut_off;             // offset of this replica's boost table in lut[]
   uint32_t lut_nb;              // entries
   uint8_t  policy, guard, signal_mode, quant_mode;
+  uint32_t pad[2];
 };
+constexpr uint32_t kWindowPad = 64;   // records allocated behind the last window (speculative chunk reads)
 
 struct SimDev {                 // kernel argument (by value)
   // configuration

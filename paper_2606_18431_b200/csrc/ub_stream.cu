@@ -5,19 +5,22 @@
 // The replica's active window is kept in HBM in the priority order of the last iteration.  MemGuard keeps keys
 // piecewise constant: between two iterations only the few requests whose (residency, bin, class)
 // changed -- listed by the previous iteration in the replica's dirty list -- and the new arrivals can change place.
-// One iteration is ONE pass over the window, 32 requests per chunk, one 16-byte record of each array per lane, the
-// next chunk in flight while the current one is processed:
+// One iteration is ONE pass over the window, 32 requests per chunk, one 16-byte record of each array per lane:
 //   a0 ingest / idle jump (M6)    arrivals are read from the packed trace
 //   a1 score (M3-M5)              boost table held in registers (lane b holds LUT[b]), looked up by shuffle
 //   a2 order                      the dirty requests and the arrivals (<= 32 together) are scored, ranked against each
 //                                 other in-warp and merged into the stream of the other, still sorted, requests
-//   a3 admit (M7)                 the walk is a carried state machine over the chunks: two warp scans per chunk
-//                                 (tokens, KV blocks), a ballot for the first misfit, "residents only" behind a
-//                                 blocked newcomer, nothing once the walk has stopped
+//   a3 admit (M7)                 the walk is a carried state machine over the chunks: a chunk that fits as a whole
+//                                 costs two warp reductions, the one holding the first misfit two warp scans and a
+//                                 ballot; "residents only" behind a blocked newcomer; nothing once the walk stopped
 //   a5 advance (M9-M10, M12)      applied in the same pass, records rewritten in place (E1 when it changed, E0 only
 //                                 where the order shifts); what needs the iteration's end time (first token, gap
 //                                 after a stall, completion) is queued and applied when the cost is known
 //   a4 victim select (M8)         if the stalled residents no longer fit: one backward pass over the window tail
+// Data movement: every global -> SM transfer of the window is asynchronous (cp.async, 16 bytes per lane, L2 only)
+// into per-warp shared-memory stages.  While a warp works on replica r it already has the header, the parameters,
+// the dirty list and the first two chunks of its NEXT replica in flight, and a ring of kRing chunks of r ahead of the
+// one it is processing; no register holds data in flight.
 // Integers only.  Not handled here, decided before any write and queued for the team kernels of ub_step.cu: the
 // SRPT / LAS keys (they drift every token), the test-only signal / quantiser modes, a block size that is not a power
 // of two, more than 32 dirty requests + arrivals in one iteration.
@@ -26,6 +29,7 @@
 namespace ub {
 
 constexpr int kSWarps = 4;                 // warps per CTA, each streams its own replicas
+constexpr int kRing = 4;                   // chunks in flight behind the two speculative ones
 constexpr uint32_t kFull = 0xffffffffu;
 
 // inclusive warp scan, one SHFL + one predicated add per step (the shuffle's own "source lane in range" predicate)
@@ -38,11 +42,22 @@ __device__ __forceinline__ uint32_t scan32(uint32_t v) {
   return v;
 }
 
-struct __align__(16) SideStash {           // per warp: the dirty requests + arrivals of one iteration, in key order
-  uint4 r0[32];
-  uint4 r1[32];
-  uint4 kb[32];                            // {key lo, key hi, bin, -}
-};
+__device__ __forceinline__ void cp16(void* smem, const void* gmem) {
+  const uint32_t sa = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+
+struct __align__(16) WarpBuf {             // per warp, 10 KB
+  uint4 spec[2][2][64];                    // [parity][chunk 0 / 1][E0 records 0..31 | E1 records 32..63] of a replica
+  uint4 ring[kRing][64];                   // chunks 2, 3, ... of the current replica
+  uint4 hdr[2][10];                        // Hdr (160 bytes)
+  uint4 par[2][2];                         // RepPar (32 bytes)
+  uint4 dl[2][4];                          // dirty list (32 x u16)
+  uint4 sr0[32], sr1[32], skb[32];         // the dirty requests + arrivals of one iteration in key order;
+};                                         // skb = {key lo, key hi, bin, -}
+static_assert(sizeof(RepPar) == 32 && sizeof(Hdr) == 160, "cp.async copies these as 16-byte pieces");
 
 // a1 (M3-M5): sig = P + d; bin = Eq. 8 exponent; pi = a - b_gamma(w_hat) - delta if
 // resident (Eq. 7); key = class<<63 | (pi + 2^62); class 0 = MemGuard-locked resident.  All 32 lanes must call it.
@@ -62,41 +77,50 @@ __device__ __forceinline__ void score(const Rec0& q0, const Rec1& q1, uint32_t k
 }
 
 __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
-  __shared__ SideStash stash[kSWarps];
+  __shared__ WarpBuf wbuf[kSWarps];
   const SimDev& s = A.s;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const uint32_t ltmask = (1u << lane) - 1u;
-  SideStash& X = stash[wib];
+  WarpBuf& X = wbuf[wib];
   const uint32_t B = s.B, M = s.M, cc = s.c, Tb = s.T, Q = s.Q, k = s.k;
   const uint32_t blk_m1 = s.blk - 1u, blk_sh = s.blk_shift;
   const uint32_t nwarps = gridDim.x * kSWarps;
 
-  for (uint32_t r = blockIdx.x * kSWarps + wib; r < s.R; r += nwarps) {
-    // ---- everything whose address depends on r only is requested at once: header words (Hdr, ub_internal.cuh;
-    // uniform loads), parameters, the first chunk of the window and the dirty list (speculatively)
-    unsigned long long* h64 = reinterpret_cast<unsigned long long*>(s.hdr + r);
-    Rec0* gE0 = s.E0 + (size_t)r * Q;
-    Rec1* gE1 = s.E1 + (size_t)r * Q;
-    const unsigned long long w13 = __ldcg(h64 + 13);
-    int64_t a_next = (int64_t)__ldcg(h64 + 2);
-    int64_t t = (int64_t)__ldcg(h64 + 0);
-    uint64_t H = __ldcg(h64 + 1);
-    const unsigned long long w14 = __ldcg(h64 + 14);
-    uint32_t nd = (uint32_t)__ldcg(h64 + 18);                         // entries of the dirty list
-    const RepPar par = s.par[r];
-    int4 p0 = make_int4(0, 0, 0, 0), p1 = make_int4(0, 0, 0, 0);
-    if ((uint32_t)lane < Q) {
-      p0 = __ldcg(reinterpret_cast<const int4*>(gE0 + lane));
-      p1 = __ldcg(reinterpret_cast<const int4*>(gE1 + lane));
+  // header, parameters, dirty list and the first two chunks of replica rr -> stage `par` (one cp.async group)
+  auto prefetch_replica = [&](const uint32_t rr, const uint32_t par) {
+    if (rr < s.R) {
+      if (lane < 10) cp16(&X.hdr[par][lane], reinterpret_cast<const uint4*>(s.hdr + rr) + lane);
+      else if (lane < 12) cp16(&X.par[par][lane - 10], reinterpret_cast<const uint4*>(s.par + rr) + (lane - 10));
+      else if (lane < 16)
+        cp16(&X.dl[par][lane - 12], reinterpret_cast<const uint4*>(s.dlist + (size_t)rr * kDirtyMax) + (lane - 12));
+      const uint4* e0 = reinterpret_cast<const uint4*>(s.E0 + (size_t)rr * Q) + lane;
+      const uint4* e1 = reinterpret_cast<const uint4*>(s.E1 + (size_t)rr * Q) + lane;
+      cp16(&X.spec[par][0][lane], e0);        cp16(&X.spec[par][0][32 + lane], e1);
+      cp16(&X.spec[par][1][lane], e0 + 32);   cp16(&X.spec[par][1][32 + lane], e1 + 32);   // (arrays are padded)
     }
-    uint32_t pdl = __ldcg(s.dlist + (size_t)r * kDirtyMax + lane);
+    cp_commit();
+  };
+
+  uint32_t r = blockIdx.x * kSWarps + wib;
+  uint32_t parity = 0;
+  prefetch_replica(r, 0);
+  for (; r < s.R; r += nwarps, parity ^= 1u) {
+    cp_wait<0>();
+    __syncwarp();
+    prefetch_replica(r + nwarps, parity ^ 1u);
+    const unsigned long long* sh = reinterpret_cast<const unsigned long long*>(X.hdr[parity]);
+    unsigned long long* h64 = reinterpret_cast<unsigned long long*>(s.hdr + r);
+    const unsigned long long w13 = sh[13];
+    int64_t a_next = (int64_t)sh[2];
     uint32_t n = (uint32_t)w13, next = (uint32_t)(w13 >> 32);
     if (n == 0 && a_next == kNever) continue;                         // finished its trace
-    uint32_t swap_used = (uint32_t)w14, peak = (uint32_t)(w14 >> 32);
+    int64_t t = (int64_t)sh[0];
+    uint32_t nd = (uint32_t)sh[18];                                   // entries of the dirty list
     const uint32_t iters = A.iters;
-
+    const RepPar par = *reinterpret_cast<const RepPar*>(X.par[parity]);
     const Rec0* TR = s.TR + (size_t)par.trace_id * s.N;
-    uint16_t* gdl = s.dlist + (size_t)r * kDirtyMax;
+    Rec0* gE0 = s.E0 + (size_t)r * Q;
+    Rec1* gE1 = s.E1 + (size_t)r * Q;
     const bool isboost = par.policy == 2;
     const int64_t delta = par.delta;
     const bool guard = par.guard != 0;
@@ -126,7 +150,29 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       wsize = n + cnt;
       if (nd + cnt > kDirtyMax) { slow = true; break; }               // (nd > kDirtyMax marks a list that overflowed)
       const uint32_t n_old = n, m = nd + cnt;
+      const uint32_t nch = (n_old + 31u) >> 5;
       n += cnt;
+
+      // chunks 2 .. of the window: kRing cp.async groups in flight (group q of the ring = chunk 2 + q, maybe empty)
+      auto issue_chunk = [&](const uint32_t c) {
+        if (c < nch) {
+          uint4* st = X.ring[(c - 2u) % kRing];
+          cp16(st + lane, reinterpret_cast<const uint4*>(gE0 + c * 32u) + lane);
+          cp16(st + 32 + lane, reinterpret_cast<const uint4*>(gE1 + c * 32u) + lane);
+        }
+        cp_commit();
+      };
+      if (it > 0) {                                                   // (the first iteration found them prefetched)
+        cp16(&X.spec[parity][0][lane], reinterpret_cast<const uint4*>(gE0) + lane);
+        cp16(&X.spec[parity][0][32 + lane], reinterpret_cast<const uint4*>(gE1) + lane);
+        cp16(&X.spec[parity][1][lane], reinterpret_cast<const uint4*>(gE0) + 32 + lane);
+        cp16(&X.spec[parity][1][32 + lane], reinterpret_cast<const uint4*>(gE1) + 32 + lane);
+        cp_commit();
+      }
+      if (nch > 2u) {
+#pragma unroll
+        for (int q = 0; q < kRing; q++) issue_chunk(2u + q);
+      }
 
       // ---------------- a2 (first half): the requests that may change place -- dirty ones and arrivals -- are taken
       // out of the stream, scored, ranked among themselves by (class, key, id) and parked in shared memory
@@ -134,7 +180,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       if (m) {
         int4 v0 = make_int4(0, 0, 0, 0), v1 = make_int4(0, 0, 0, 0);
         if ((uint32_t)lane < nd) {
-          spos = pdl;
+          spos = it == 0 ? (uint32_t)reinterpret_cast<const uint16_t*>(X.dl[parity])[lane]
+                         : (uint32_t)__ldcg(s.dlist + (size_t)r * kDirtyMax + lane);
           v0 = __ldcg(reinterpret_cast<const int4*>(gE0 + spos));
           v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + spos));
         } else if ((uint32_t)lane < m) {
@@ -159,16 +206,17 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           }
         }
         if ((uint32_t)lane < m) {
-          X.r0[rank] = *reinterpret_cast<const uint4*>(&v0);
-          X.r1[rank] = *reinterpret_cast<const uint4*>(&v1);
-          X.kb[rank] = make_uint4((uint32_t)sk, (uint32_t)(sk >> 32), sb, 0u);
+          X.sr0[rank] = *reinterpret_cast<const uint4*>(&v0);
+          X.sr1[rank] = *reinterpret_cast<const uint4*>(&v1);
+          X.skb[rank] = make_uint4((uint32_t)sk, (uint32_t)(sk >> 32), sb, 0u);
         }
-        __syncwarp();
       }
+      if (it > 0) { if (nch > 2u) cp_wait<kRing>(); else cp_wait<0>(); }   // the re-read chunks 0, 1
+      __syncwarp();
 
       // ---------------- the pass.  Walk state (M7), warp-uniform: mode 0 = everybody walks, 1 = residents only (a
       // newcomer was blocked on KV), 2 = stopped; carryW / carryC = tokens / KV blocks claimed so far; crank = rank of
-      // the next request in the merged order; carryN = requests admitted so far (mode 1).
+      // the next request in the merged order (mode 0); carryN = requests admitted so far (mode 1).
       uint32_t mode = 0, carryW = 0, carryC = 0, carryN = 0, crank = 0;
       uint32_t pf = 0, dec = 0, kres = 0, evl = 0, evu = 0, emit = 0, same = 0, swb = 0, swc = 0;   // per-lane sums
       uint32_t outpos = 0, nev = 0, ndnew = 0, n_done = 0;
@@ -182,7 +230,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const bool res = valid && (of & F_RESIDENT) != 0;
         const uint32_t rem = w0.P + w1.d - w1.cached;
         uint32_t want = 0;
-        // ---- a3: admission walk as prefix scans (M7; Algorithm 1 "while |B| < M ... U + dU <= B")
+        // ---- a3: admission walk (M7; Algorithm 1 "while |B| < M ... U + dU <= B") over this segment:
         //   W = incl. scan of min(c, rem);  tok_before = min(T, W - w);  want = min(T, W) - tok_before;
         //   foot = ceil((cached + want)/blk);  Cf = incl. scan of foot;  ok = rank < M & tok_before < T & Cf <= B.
         // ok is monotone along the walk: the admitted set is the prefix in front of the first misfit.  If that one is
@@ -190,41 +238,50 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         if (mode < 2u) {
           const uint32_t resm = __ballot_sync(kFull, res);
           uint32_t pm = mode == 0u ? mask : resm;
-          uint32_t from = 0;                                          // lanes below `from` are settled
-          while (pm) {                                                // at most two rounds per segment
-            const bool part = (pm >> lane) & 1u;
-            const uint32_t w = part ? (rem < cc ? rem : cc) : 0u;
-            const uint32_t W = carryW + scan32(w);
-            const uint32_t tok_before = (W - w) < Tb ? (W - w) : Tb;
-            const uint32_t tok_after = W < Tb ? W : Tb;
-            const uint32_t wnt = tok_after - tok_before;
-            const uint32_t foot = part ? (w1.cached + wnt + blk_m1) >> blk_sh : 0u;
-            const uint32_t Cf = carryC + scan32(foot);
-            const uint32_t cb = (mode == 0u ? crank : carryN) + __popc(pm & ltmask);
-            const bool ok = part && cb < M && tok_before < Tb && Cf <= B;
-            if (ok) want = wnt;
-            const uint32_t fm = __ballot_sync(kFull, part && !ok);
-            if (!fm) {
-              carryW = __shfl_sync(kFull, W, 31);
-              carryC = __shfl_sync(kFull, Cf, 31);
-              carryN += __popc(pm);
-              break;
-            }
-            const int fl = __ffs(fm) - 1;                             // the first request that did not fit
-            const uint32_t fC = __shfl_sync(kFull, Cf - foot, fl);
-            const uint32_t ftok = __shfl_sync(kFull, tok_before, fl);
-            const uint32_t fcb = __shfl_sync(kFull, cb, fl);
-            carryC = fC; carryW = ftok; carryN = fcb;
-            if (mode == 0u && fcb < M && ftok < Tb && !((resm >> fl) & 1u)) {
-              mode = 1u;                                              // newblocked: residents behind it continue
-              from = (uint32_t)fl + 1u;
-              pm = from < 32u ? (resm & (kFull << from)) : 0u;
+          if (pm) {
+            const bool part0 = (pm >> lane) & 1u;
+            const uint32_t w0t = part0 ? (rem < cc ? rem : cc) : 0u;
+            const uint32_t f0 = part0 ? (w1.cached + w0t + blk_m1) >> blk_sh : 0u;
+            const uint32_t totw = __reduce_add_sync(kFull, w0t);
+            const uint32_t totf = __reduce_add_sync(kFull, f0);
+            const uint32_t npm = __popc(pm);
+            if (carryW + totw <= Tb && carryC + totf <= B && (mode == 0u ? crank : carryN) + npm <= M) {
+              want = w0t;                                             // the whole segment fits: no misfit in it
+              carryW += totw; carryC += totf; carryN += npm;
             } else {
-              mode = 2u;
-              pm = 0u;
+              while (pm) {                                            // at most two rounds per segment
+                const bool part = (pm >> lane) & 1u;
+                const uint32_t w = part ? w0t : 0u;
+                const uint32_t W = carryW + scan32(w);
+                const uint32_t tok_before = (W - w) < Tb ? (W - w) : Tb;
+                const uint32_t tok_after = W < Tb ? W : Tb;
+                const uint32_t wnt = tok_after - tok_before;
+                const uint32_t foot = part ? (w1.cached + wnt + blk_m1) >> blk_sh : 0u;
+                const uint32_t Cf = carryC + scan32(foot);
+                const uint32_t cb = (mode == 0u ? crank : carryN) + __popc(pm & ltmask);
+                const bool ok = part && cb < M && tok_before < Tb && Cf <= B;
+                if (ok) want = wnt;
+                const uint32_t fm = __ballot_sync(kFull, part && !ok);
+                if (!fm) {
+                  carryW = __shfl_sync(kFull, W, 31);
+                  carryC = __shfl_sync(kFull, Cf, 31);
+                  carryN += __popc(pm);
+                  break;
+                }
+                const int fl = __ffs(fm) - 1;                         // the first request that did not fit
+                carryC = __shfl_sync(kFull, Cf - foot, fl);
+                carryW = __shfl_sync(kFull, tok_before, fl);
+                carryN = __shfl_sync(kFull, cb, fl);
+                if (mode == 0u && carryN < M && carryW < Tb && !((resm >> fl) & 1u)) {
+                  mode = 1u;                                          // newblocked: residents behind it continue
+                  pm = fl < 31 ? (resm & (kFull << (fl + 1))) : 0u;
+                } else {
+                  mode = 2u;
+                  pm = 0u;
+                }
+              }
             }
           }
-          (void)from;
         }
         crank += __popc(mask);
 
@@ -278,7 +335,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const bool defer = emitted && (d_old == 0u || !ep_old || gone);
         const bool ends = valid && !emitted && ep_old;
         if (__any_sync(kFull, defer || ends)) {
-          if (ends) s.t_last[(size_t)r * s.N + w1.id] = t;                               // persist t_last when the streak ends
+          if (ends) s.t_last[(size_t)r * s.N + w1.id] = t;            // persist t_last when the streak ends
           const uint32_t em = __ballot_sync(kFull, defer);
           if (defer)
             s.evbuf[(size_t)r * s.evcap + nev + __popc(em & ltmask)] =
@@ -297,50 +354,48 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const uint32_t dm = __ballot_sync(kFull, keep && dirty);
         if (dm) {                                                     // next iteration's dirty list
           const uint32_t slot = ndnew + __popc(dm & ltmask);
-          if (keep && dirty && slot < kDirtyMax) gdl[slot] = (uint16_t)np;
+          if (keep && dirty && slot < kDirtyMax) s.dlist[(size_t)r * kDirtyMax + slot] = (uint16_t)np;
           ndnew += __popc(dm);
         }
         outpos += __popc(keepm);
         n_done += __popc(gonem);
       };
 
-      const uint32_t nch = (n_old + 31u) >> 5;
-      int4 nx0 = make_int4(0, 0, 0, 0), nx1 = make_int4(0, 0, 0, 0);
-      if ((uint32_t)lane < n_old) { nx0 = p0; nx1 = p1; }
       for (uint32_t c = 0; c <= nch; c++) {
         if (c == nch && dptr >= m) break;                             // (chunk nch is empty: the parked tail)
-        const int4 c0 = nx0, c1 = nx1;
-        {
-          const uint32_t pn = (c + 1u) * 32u + (uint32_t)lane;
-          nx0 = make_int4(0, 0, 0, 0); nx1 = make_int4(0, 0, 0, 0);
-          if (pn < n_old) {
-            nx0 = __ldcg(reinterpret_cast<const int4*>(gE0 + pn));
-            nx1 = __ldcg(reinterpret_cast<const int4*>(gE1 + pn));
-          }
-        }
+        // the chunk must have landed; when parked requests are merged in, the writes of this chunk may reach into
+        // the next one, which must then have landed too before anything is stored
+        if (c >= 2u) { if (m) cp_wait<kRing - 2>(); else cp_wait<kRing - 1>(); __syncwarp(); }
+        else if (c == 1u && m && nch > 2u) { cp_wait<kRing - 1>(); __syncwarp(); }
+        const uint4* st = c < 2u ? X.spec[parity][c] : X.ring[(c - 2u) % kRing];
+        const uint4 c0 = st[lane], c1 = st[32 + lane];
+        if (c >= 2u) { __syncwarp(); issue_chunk(c + kRing); }        // the stage is free again
         const Rec0 r0 = *reinterpret_cast<const Rec0*>(&c0);
         const Rec1 r1 = *reinterpret_cast<const Rec1*>(&c1);
         const uint32_t left = c < nch ? n_old - c * 32u : 0u;
         uint32_t cv = left >= 32u ? kFull : ((1u << left) - 1u);      // requests of this chunk still in the stream
+        if (nd) cv &= ~__reduce_or_sync(kFull, ((uint32_t)lane < nd && (spos >> 5) == c) ? (1u << (spos & 31u)) : 0u);
+        if (mode == 2u && dptr >= m) {
+          // ---- behind the walk: a chunk of waiting requests (not resident, nothing to finalise) only moves up
+          const bool steady = (r1.flags & ~F_SWAPPED) == F_KLASS1;
+          if (__all_sync(kFull, steady || !((cv >> lane) & 1u))) {
+            const uint32_t np = outpos + __popc(cv & ltmask);
+            if (np != c * 32u + (uint32_t)lane && ((cv >> lane) & 1u)) {
+              __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
+              __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
+            }
+            outpos += __popc(cv);
+            continue;
+          }
+        }
         uint64_t key; uint32_t bin;
         score(r0, r1, k, lutv, delta, guard, key, bin);
-        if (m) {
-          if (nd)
-            cv &= ~__reduce_or_sync(kFull, ((uint32_t)lane < nd && (spos >> 5) == c) ? (1u << (spos & 31u)) : 0u);
-          // writes of this chunk may reach into the next one when parked requests are merged in front of it: the
-          // next chunk must have arrived in registers before anything is stored
-          uint32_t dummy;
-          asm volatile("{ .reg .pred p; setp.eq.u32 p, %1, %2; vote.sync.ballot.b32 %0, p, 0xffffffff; }"
-                       : "=r"(dummy) : "r"(nx0.x), "r"(nx1.w) : "memory");
-          (void)dummy;
-          __syncwarp();
-        }
         uint32_t lo = 0;
         for (;;) {
           uint32_t fl = 32;
           if (dptr < m) {                                             // clean requests that sort behind the next parked one
-            const uint4 dk = X.kb[dptr];
-            const uint32_t di = X.r1[dptr].x;
+            const uint4 dk = X.skb[dptr];
+            const uint32_t di = X.sr1[dptr].x;
             const uint32_t after = __ballot_sync(kFull, ((cv >> lane) & 1u) && (uint32_t)lane >= lo &&
                                                  key_less((uint64_t)dk.x | ((uint64_t)dk.y << 32), di, key, r1.id));
             if (after) fl = (uint32_t)__ffs(after) - 1u;
@@ -353,13 +408,13 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           if (fl < 32u) {
             const uint64_t ck = __shfl_sync(kFull, key, (int)fl);
             const uint32_t ci = __shfl_sync(kFull, r1.id, (int)fl);
-            const uint4 kb = X.kb[lane];
+            const uint4 kb = X.skb[lane];
             j = __popc(__ballot_sync(kFull, (uint32_t)lane >= dptr && (uint32_t)lane < m &&
-                                     key_less((uint64_t)kb.x | ((uint64_t)kb.y << 32), X.r1[lane].x, ck, ci)));
+                                     key_less((uint64_t)kb.x | ((uint64_t)kb.y << 32), X.sr1[lane].x, ck, ci)));
           }
           {
             const uint32_t src = dptr + (uint32_t)lane < 32u ? dptr + (uint32_t)lane : 31u;
-            const uint4 a0 = X.r0[src], a1 = X.r1[src], ak = X.kb[src];
+            const uint4 a0 = X.sr0[src], a1 = X.sr1[src], ak = X.skb[src];
             process(*reinterpret_cast<const Rec0*>(&a0), *reinterpret_cast<const Rec1*>(&a1),
                     (uint64_t)ak.x | ((uint64_t)ak.y << 32), ak.z, j < 32u ? ((1u << j) - 1u) : kFull, 0xFFFFFFFFu);
           }
@@ -374,6 +429,9 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       dec = de & 0xFFFFu; emit = de >> 16;
       same = __reduce_add_sync(kFull, same);
       kres = __reduce_add_sync(kFull, kres);
+      const unsigned long long w14 = reinterpret_cast<const unsigned long long*>(X.hdr[parity])[14];
+      uint32_t swap_used = (uint32_t)w14;
+      const uint32_t peak = (uint32_t)(w14 >> 32);
       uint32_t swin_blocks = 0, swin_cnt = 0;
       if (__any_sync(kFull, swc != 0u)) {
         swin_blocks = __reduce_add_sync(kFull, swb);
@@ -436,7 +494,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           const uint32_t dm = __ballot_sync(kFull, victim && !(of & F_DIRTY));      // residency changed => dirty
           if (dm) {
             const uint32_t slot = ndnew + __popc(dm & ltmask);
-            if (victim && !(of & F_DIRTY) && slot < kDirtyMax) gdl[slot] = (uint16_t)pos;
+            if (victim && !(of & F_DIRTY) && slot < kDirtyMax) s.dlist[(size_t)r * kDirtyMax + slot] = (uint16_t)pos;
             ndnew += __popc(dm);
           }
           behind += tot;
@@ -485,16 +543,20 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       evu = __reduce_add_sync(kFull, evu);
 
       // ---------------- header: clock, digest (M12), cursors; counters by RED (no read needed)
-      H = digest_fold(H, evl, evu, t_end);
       if (ndnew > kDirtyMax) ndnew = kDirtyMax + 1u;
       if (lane == 0) {
+        unsigned long long* shw = reinterpret_cast<unsigned long long*>(X.hdr[parity]);
+        const uint64_t H = digest_fold(shw[1], evl, evu, t_end);
+        shw[1] = H;                                                   // (kept current for a further iteration)
+        const uint32_t pk = n > peak ? n : peak;
+        shw[14] = (unsigned long long)swap_used | ((unsigned long long)pk << 32);
         if (same) atomicAdd(s.hist + (size_t)r * kTbtBins + tbt_bin(cost), same);
         __stcg(h64 + 0, (unsigned long long)t_end);
         __stcg(h64 + 1, (unsigned long long)H);
         if (cnt) __stcg(h64 + 2, (unsigned long long)a_next);
         __stcg(h64 + 13, (unsigned long long)n_new | ((unsigned long long)next << 32));
         if (n > peak || swin_blocks || swout_blocks)
-          __stcg(h64 + 14, (unsigned long long)swap_used | ((unsigned long long)(n > peak ? n : peak) << 32));
+          __stcg(h64 + 14, (unsigned long long)swap_used | ((unsigned long long)pk << 32));
         if (ndnew != nd) __stcg(reinterpret_cast<uint32_t*>(h64 + 18), ndnew);
         atomicAdd(h64 + 3, (unsigned long long)n);                    // request-steps
         atomicAdd(h64 + 4, (unsigned long long)emit);
@@ -505,7 +567,6 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         if (n_done | ev_nrc) atomicAdd(h64 + 15, (unsigned long long)n_done | ((unsigned long long)ev_nrc << 32));
         if (ev_nsw | swin_cnt) atomicAdd(h64 + 16, (unsigned long long)ev_nsw | ((unsigned long long)swin_cnt << 32));
       }
-      if (n > peak) peak = n;
       t = t_end; n = n_new; wsize = n_new; nd = ndnew;
       if (n == 0 && a_next == kNever) {                               // finished its trace in this call
         if (lane == 0) atomicAdd(A.count + 5, 1u);
@@ -513,13 +574,6 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         break;
       }
       __syncwarp();                                                   // window stores before the next iteration's loads
-      if (it + 1u < iters) {
-        if ((uint32_t)lane < Q) {
-          p0 = __ldcg(reinterpret_cast<const int4*>(gE0 + lane));
-          p1 = __ldcg(reinterpret_cast<const int4*>(gE1 + lane));
-        }
-        pdl = __ldcg(gdl + lane);
-      }
     }
 
     // ---------------- not handled here: queue the replica for the team kernels of this round
@@ -528,12 +582,14 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       push_list(A, wsize <= A.thrS ? 0u : (wsize <= A.thrM ? 1u : 2u), r);
     }
   }
+  cp_wait<0>();
 }
 
 // persistent grid: every warp strides over the replicas
 void launch_stream(const StepArgs& A, cudaStream_t st) {
   static int ctas_per_sm = 0;
   if (!ctas_per_sm) {
+    cudaFuncSetAttribute(k_stream, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream, 32 * kSWarps, 0) != cudaSuccess ||
         ctas_per_sm < 1)
       ctas_per_sm = 4;
