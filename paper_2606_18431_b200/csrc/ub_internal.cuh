@@ -27,6 +27,7 @@ constexpr uint32_t F_DIRTY    = 8u;        // (class,key) may differ from the pr
 constexpr uint32_t F_ADMITNOW = 16u;       // admitted in the last executed iteration (read by the eviction pass only)
 constexpr uint32_t F_KLASS1   = 32u;       // was in class 1 (not MemGuard-locked) in the last executed iteration
 constexpr int      F_LOCK_SHIFT = 6;       // bits 6..31: lockbin + 1 (0 = no lock)
+constexpr uint32_t F_LOCK_MASK_LOW = (1u << F_LOCK_SHIFT) - 1u;   // the flag bits below the lock field
 constexpr uint32_t kDirtyMax  = 32;        // entries of a replica's dirty list; Hdr::n_dirty > kDirtyMax = overflow
 
 struct __align__(16) Rec0 { int64_t a; uint32_t P; uint32_t D; };

@@ -388,6 +388,34 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
             continue;
           }
         }
+        if (mode == 0u && dptr >= m && guard) {
+          // ---- a chunk of MemGuard-locked residents in steady decode (each wants one token, emits it, neither
+          // completes nor crosses its Eq. 8 threshold) that fits as a whole: class 0 in stored order, nothing is
+          // re-keyed, every record just advances by one token (M2, M7, M10)
+          const bool valid = (cv >> lane) & 1u;
+          const uint32_t fl = r1.flags;
+          const uint32_t sig1 = r0.P + r1.d + 1u;                      // signal after this token
+          const bool okl = (fl & (F_LOCK_MASK_LOW)) == (F_RESIDENT | F_ADMITNOW | F_EMITPREV) && r1.cached + 2u == sig1 &&
+                           r1.d + 1u != r0.D && sig1 != (k << (fl >> F_LOCK_SHIFT));
+          if (__all_sync(kFull, okl || !valid)) {
+            const uint32_t nv = __popc(cv);
+            const uint32_t totf = __reduce_add_sync(kFull, valid ? (r1.cached + 1u + blk_m1) >> blk_sh : 0u);
+            if (crank + nv <= M && carryW + nv <= Tb && carryC + totf <= B) {
+              const uint32_t np = outpos + __popc(cv & ltmask);
+              if (valid) {
+                if (np != c * 32u + (uint32_t)lane)
+                  __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
+                __stcg(reinterpret_cast<int4*>(gE1 + np),
+                       make_int4((int)r1.id, (int)(r1.d + 1u), (int)(r1.cached + 1u), (int)fl));
+                const uint64_t h = (uint64_t)(((r1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu)) * 3ull;
+                evl += (uint32_t)h; evu += (uint32_t)(h >> 32);
+                dec++; emit++; same++;
+              }
+              crank += nv; carryW += nv; carryC += totf; outpos += nv;
+              continue;
+            }
+          }
+        }
         uint64_t key; uint32_t bin;
         score(r0, r1, k, lutv, delta, guard, key, bin);
         uint32_t lo = 0;
