@@ -375,7 +375,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const uint32_t left = c < nch ? n_old - c * 32u : 0u;
         uint32_t cv = left >= 32u ? kFull : ((1u << left) - 1u);      // requests of this chunk still in the stream
         if (nd) cv &= ~__reduce_or_sync(kFull, ((uint32_t)lane < nd && (spos >> 5) == c) ? (1u << (spos & 31u)) : 0u);
-        if (mode == 2u && dptr >= m) {
+        if (mode != 0u && dptr >= m) {
           // ---- behind the walk: a chunk of waiting requests (not resident, nothing to finalise) only moves up
           const bool steady = (r1.flags & ~F_SWAPPED) == F_KLASS1;
           if (__all_sync(kFull, steady || !((cv >> lane) & 1u))) {
