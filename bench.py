@@ -6,10 +6,12 @@ requests, 50/50 chat/reasoning mix, Poisson arrivals at 95 % load, KV capacity 1
 BOOST gamma = 0.3, swap-vs-recompute preemption; seeded synthetic traces (workloads.config5).
 
 A "step" is one ub_step(h, ITERS) call: every replica advances ITERS scheduler iterations, each iteration one
-launch of the step kernel that streams the replica's window HBM -> SM -> HBM (all of a0..a5).  Before the timed
-region every replica is advanced SPINUP iterations (not timed) so that queues are populated.  The timed region is
-K steps on the device (CUDA events, barrier + synchronize on both sides, max over ranks).  Inputs per launch
-(~0.5 GB at n_mean ~ 200) are larger than L2 (126 MB), so no explicit flush is needed.
+launch of the streaming step kernel ub::k_stream (all of a0..a5: the replica's window goes HBM -> SM -> HBM once)
+followed by the four team-kernel launches that take what it queued (none in this config).  Before the timed
+region every replica is advanced SPINUP iterations (not timed, default 65536 = the middle of the ~1.4e5
+iterations a config-5 replica runs) so that the queues are in their loaded regime.  The timed region is K steps on
+the device (CUDA events, barrier + synchronize on both sides, max over ranks).  The windows read per launch
+(~0.4 GB) are larger than L2 (126 MB), so no explicit flush is needed.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 """
@@ -31,6 +33,8 @@ if ROOT not in sys.path:
 
 from paper_2606_18431_b200 import workloads as W  # noqa: E402
 
+KERNELS_PER_ROUND = 5                # ub::k_stream + the L, M, S and overflow launches of ub::k_step (csrc/ub_step.cu)
+TRAFFIC_BYTES_PER_LAUNCH = 483.7e6   # dram read+write bytes of one ub::k_stream launch, profiles/r01c_stream.md (ncu --set full)
 ALG_BYTES_PER_REQUEST_STEP = 40      # read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
 METRIC = "request-steps scheduled/sec"
 UNIT = "request-steps/s"
@@ -42,12 +46,12 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--iters", type=int, default=16, help="scheduler iterations per step")
-    ap.add_argument("--spinup", type=int, default=6144, help="untimed iterations before the warm-up")
+    ap.add_argument("--iters", type=int, default=64, help="scheduler iterations per step")
+    ap.add_argument("--spinup", type=int, default=65536, help="untimed iterations before the warm-up")
     ap.add_argument("--replicas", type=int, default=65536, help="replicas per GPU (config5: 65536)")
     ap.add_argument("--requests", type=int, default=8192)
     ap.add_argument("--iters-per-launch", type=int, default=1)
-    ap.add_argument("--cpu-sample", type=int, default=48, help="replicas the oracle baseline runs")
+    ap.add_argument("--cpu-sample", type=int, default=64, help="replicas the oracle baseline runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -124,7 +128,7 @@ def run_reference(args):
         return
     wl = W.config5(n_seeds=args.replicas, n_requests=args.requests)
     from oracle import oracle as O
-    ids = list(range(0, args.replicas, max(1, args.replicas // 8)))[:8]
+    ids = list(range(0, args.replicas, max(1, args.replicas // 32)))[:32]
     sub = wl.select(ids)
     o = O.OracleSim(sub.sim, sub.replicas, sub.traces())
     o.step(args.spinup)                                   # same populated-queue regime as the CUDA arm
@@ -226,7 +230,8 @@ def main():
     d2h_bytes = R * (B.C.sizeof(B.UbReplicaStats))
     ttlt_p99_us = st2[:, 14 + 3 + 2][st2[:, COL["n_completed"]] > 0]          # ttlt_us[2]
     p99 = float(np.median(ttlt_p99_us)) * 1e-6 if ttlt_p99_us.size else 0.0
-    launches = args.steps * ((args.iters + max(1, args.iters_per_launch) - 1) // max(1, args.iters_per_launch))
+    rounds = args.steps * ((args.iters + max(1, args.iters_per_launch) - 1) // max(1, args.iters_per_launch))
+    launches = rounds * KERNELS_PER_ROUND
 
     tot = torch.tensor([float(rs2 - rs1), float(rs2), ms, t_e2e], dtype=torch.float64, device="cuda")
     if world > 1:
@@ -253,9 +258,13 @@ def main():
                        "iterations_before_timed": int(it1), "l2": "inputs larger than L2 (no flush)",
                        "trace_generation_s": t_gen, "median_p99_ttlt_s": p99},
             "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                         "traffic": None, "peak_source": peak_src, "kernel": "ub::k_step",
+                         "traffic": TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src, "kernel": "ub::k_stream",
                          "alg_bytes_per_request_step": ALG_BYTES_PER_REQUEST_STEP,
-                         "avg_launch_ms": ms / max(1, launches)},
+                         "request_steps_per_launch": (rs2 - rs1) / max(1, rounds),
+                         "avg_launch_ms": ms / max(1, rounds),
+                         "note": "avg_launch_ms = timed region / scheduler rounds: one k_stream launch plus the four "
+                                 "(empty in this config) team-kernel launches, so the kernel alone is slightly faster; "
+                                 "traffic = dram read+write bytes of one k_stream launch from profiles/ (ncu --set full)"},
             "e2e": {"value": rs_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
                     "note": "one job: ub_create + ub_load_trace from pinned host + ub_set_replicas + spin-up + warm-up + timed steps + 2x ub_stats D2H; all request-steps / wall"},
             "gpu_launches": launches, "clocks": clocks,
