@@ -165,6 +165,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2606_18431_b200 import binding as B
+    from paper_2606_18431_b200 import sharding as SH
 
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -176,8 +177,7 @@ def main():
 
     # ---- synthetic traces: replicas are independent units, sharded over ranks by seed (weak scaling)
     R, N = args.replicas, args.requests
-    wl = W.config5(n_seeds=R * world, n_requests=N).select(range(rank * R, (rank + 1) * R)) if world > 1 \
-        else W.config5(n_seeds=R, n_requests=N)
+    wl = SH.shard_workload(W.config5, rank, world, R, N)
     t_gen = time.perf_counter()
     a, p, d, n = wl.traces(workers=max(1, min(32, (os.cpu_count() or 1) // max(1, world))))
     t_gen = time.perf_counter() - t_gen
@@ -233,13 +233,7 @@ def main():
     rounds = args.steps * ((args.iters + max(1, args.iters_per_launch) - 1) // max(1, args.iters_per_launch))
     launches = rounds * KERNELS_PER_ROUND
 
-    tot = torch.tensor([float(rs2 - rs1), float(rs2), ms, t_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        s_ = tot.clone(); dist.all_reduce(s_, dist.ReduceOp.SUM)
-        m_ = tot.clone(); dist.all_reduce(m_, dist.ReduceOp.MAX)
-        rs_timed, rs_all, ms, t_e2e = s_[0].item(), s_[1].item(), m_[2].item(), m_[3].item()
-    else:
-        rs_timed, rs_all = tot[0].item(), tot[1].item()
+    rs_timed, rs_all, ms, t_e2e = SH.aggregate(rs2 - rs1, rs2, ms, t_e2e, "cuda", world)
 
     if rank == 0:
         peak, peak_src = peaks()
