@@ -33,7 +33,7 @@ if ROOT not in sys.path:
 
 from paper_2606_18431_b200 import workloads as W  # noqa: E402
 
-KERNELS_PER_ROUND = 5                # ub::k_stream + the L, M, S and overflow launches of ub::k_step (csrc/ub_step.cu)
+KERNELS_PER_ROUND = 2                # ub::k_stream + the L launch of ub::k_step (every config-5 replica is stream-eligible)
 TRAFFIC_BYTES_PER_LAUNCH = 483.7e6   # dram read+write bytes of one ub::k_stream launch, profiles/r01c_stream.md (ncu --set full)
 ALG_BYTES_PER_REQUEST_STEP = 40      # read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
 METRIC = "request-steps scheduled/sec"

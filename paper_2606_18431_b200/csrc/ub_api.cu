@@ -258,6 +258,12 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
     p.policy = q.policy; p.guard = q.guard; p.signal_mode = q.signal_mode; p.quant_mode = q.quant_mode;
     p.pad[0] = p.pad[1] = 0;
   }
+  {
+    bool all = s->dev.blk_shift < 32u;
+    for (size_t r = 0; r < R && all; r++)
+      all = (reps[r].policy == UB_FCFS || reps[r].policy == UB_BOOST) && reps[r].signal_mode == 0 && reps[r].quant_mode == 0;
+    s->dev.all_stream = all ? 1u : 0u;
+  }
   cudaFree(s->d_lut); s->d_lut = nullptr;
   int rc = dmalloc(&s->d_lut, s->h_lut.size()); if (rc) return rc;
   if (!s->h_lut.empty())

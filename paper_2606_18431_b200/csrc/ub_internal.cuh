@@ -76,6 +76,7 @@ struct SimDev {                 // kernel argument (by value)
   uint16_t* dlist;              // [R][kDirtyMax] window positions of the re-keyed ("dirty") requests
   uint2*    evbuf;              // [R][evcap] scratch: per-request events of one iteration that wait for t_end
   uint32_t  evcap;              // min(M, Q)
+  uint32_t  all_stream;         // every replica is eligible for the streaming kernel: its rare hand-overs all go to the L team kernel
 };
 
 // kernels (ub_step.cu, ub_aux.cu)

@@ -703,12 +703,14 @@ void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iter
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
+  if (s.all_stream) A.thrS = A.thrM = 0;                                        // (windows are never empty when queued)
   cudaMemsetAsync(count, 0, 4 * sizeof(uint32_t), st);                          // this round's lists start empty
   launch_stream(A, st);
   const uint32_t R = s.R;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;
   const uint32_t nS = (R + kTeamsS - 1) / kTeamsS, gS = nS < 148u * 10 ? nS : 148u * 10;
   k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 2u, 0xFFFFFFFFu);
+  if (s.all_stream) return;                      // nothing can be queued for the smaller teams
   k_step<4, kEM, 1><<<gM, 128, TeamSmem<4, kEM>::BYTES, st>>>(A, 1u, 0xFFFFFFFFu);
   k_step<1, kES, kTeamsS><<<gS, 32 * kTeamsS, kTeamsS * TeamSmem<1, kES>::BYTES, st>>>(A, 0u, 0xFFFFFFFFu);
   k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 3u, 0xFFFFFFFFu);

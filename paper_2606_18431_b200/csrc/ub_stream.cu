@@ -375,23 +375,40 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const uint32_t left = c < nch ? n_old - c * 32u : 0u;
         uint32_t cv = left >= 32u ? kFull : ((1u << left) - 1u);      // requests of this chunk still in the stream
         if (nd) cv &= ~__reduce_or_sync(kFull, ((uint32_t)lane < nd && (spos >> 5) == c) ? (1u << (spos & 31u)) : 0u);
-        if (mode != 0u && dptr >= m) {
+        // the next parked request, if any: fast paths apply only to chunks that sort in front of it
+        const bool pend = dptr < m;
+        uint32_t pk_lo = 0, pk_hi = 0, pk_id = 0;
+        if (pend) { const uint4 dk = X.skb[dptr]; pk_lo = dk.x; pk_hi = dk.y; pk_id = X.sr1[dptr].x; }
+        uint64_t key = 0; uint32_t bin = 0;
+        bool scored = false;
+        if (mode != 0u && cv != 0u) {
           // ---- behind the walk: a chunk of waiting requests (not resident, nothing to finalise) only moves up
           const bool steady = (r1.flags & ~F_SWAPPED) == F_KLASS1;
           if (__all_sync(kFull, steady || !((cv >> lane) & 1u))) {
-            const uint32_t np = outpos + __popc(cv & ltmask);
-            if (np != c * 32u + (uint32_t)lane && ((cv >> lane) & 1u)) {
-              __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
-              __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
+            bool before = true;
+            if (pend) {
+              score(r0, r1, k, lutv, delta, guard, key, bin);
+              scored = true;
+              const int last = 31 - __clz((int)cv);
+              const uint64_t lk = __shfl_sync(kFull, key, last);
+              const uint32_t li = __shfl_sync(kFull, r1.id, last);
+              before = key_less(lk, li, (uint64_t)pk_lo | ((uint64_t)pk_hi << 32), pk_id);
             }
-            outpos += __popc(cv);
-            continue;
+            if (before) {
+              const uint32_t np = outpos + __popc(cv & ltmask);
+              if (np != c * 32u + (uint32_t)lane && ((cv >> lane) & 1u)) {
+                __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
+                __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
+              }
+              outpos += __popc(cv);
+              continue;
+            }
           }
         }
-        if (mode == 0u && dptr >= m && guard) {
+        if (mode == 0u && guard && cv != 0u && (!pend || (pk_hi >> 31))) {
           // ---- a chunk of MemGuard-locked residents in steady decode (each wants one token, emits it, neither
-          // completes nor crosses its Eq. 8 threshold) that fits as a whole: class 0 in stored order, nothing is
-          // re-keyed, every record just advances by one token (M2, M7, M10)
+          // completes nor crosses its Eq. 8 threshold) that fits as a whole: class 0 in stored order (so in front of
+          // a parked request of class 1), nothing is re-keyed, every record advances by one token (M2, M7, M10)
           const bool valid = (cv >> lane) & 1u;
           const uint32_t fl = r1.flags;
           const uint32_t sig1 = r0.P + r1.d + 1u;                      // signal after this token
@@ -416,8 +433,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
             }
           }
         }
-        uint64_t key; uint32_t bin;
-        score(r0, r1, k, lutv, delta, guard, key, bin);
+        if (!scored) score(r0, r1, k, lutv, delta, guard, key, bin);
         uint32_t lo = 0;
         for (;;) {
           uint32_t fl = 32;
@@ -607,7 +623,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     // ---------------- not handled here: queue the replica for the team kernels of this round
     if (slow && lane == 0) {
       if (it > 0) reinterpret_cast<uint32_t*>(h64 + 17)[1] = iters - it;       // iterations still to do
-      push_list(A, wsize <= A.thrS ? 0u : (wsize <= A.thrM ? 1u : 2u), r);
+      push_list(A, s.all_stream ? 2u : (wsize <= A.thrS ? 0u : (wsize <= A.thrM ? 1u : 2u)), r);
     }
   }
   cp_wait<0>();
