@@ -38,7 +38,7 @@ void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, 
 }
 
 // ------------------------------------------------------------------ reset (ub_set_replicas)
-// count[0..3] = work lists of the current round, count[5] = replicas that have finished their trace
+// count[0..3] = work lists of the current round, count[4] = k_stream's ticket counter, count[5] = replicas that have finished their trace
 __global__ void k_reset(SimDev s, uint32_t* count) {
   const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= s.R) return;

@@ -704,7 +704,7 @@ void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iter
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
   if (s.all_stream) A.thrS = A.thrM = 0;                                        // (windows are never empty when queued)
-  cudaMemsetAsync(count, 0, 4 * sizeof(uint32_t), st);                          // this round's lists start empty
+  cudaMemsetAsync(count, 0, 5 * sizeof(uint32_t), st);                          // this round's lists and ticket counter
   launch_stream(A, st);
   const uint32_t R = s.R;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;

@@ -101,13 +101,23 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     cp_commit();
   };
 
-  uint32_t r = blockIdx.x * kSWarps + wib;
+  // Work distribution: windows differ by two orders of magnitude.  A warp takes its first `nstat` replicas by static
+  // striding (3/4 of an even share); the rest are handed out dynamically: each is the next value of a global ticket
+  // counter (count[4], zeroed per round), requested one replica ahead so that the atomic's latency is never waited for.
+  const uint32_t gw = blockIdx.x * kSWarps + wib;
+  const uint32_t share = (s.R / nwarps) * 3u / 4u;
+  const uint32_t nstat = share > 2u ? share : 2u;
+  const uint32_t dynbase = nstat * nwarps;
+  uint32_t r = gw, rn = gw + nwarps;
+  uint32_t taken = 2, ticket = 0;
   uint32_t parity = 0;
   prefetch_replica(r, 0);
-  for (; r < s.R; r += nwarps, parity ^= 1u) {
+  for (; r < s.R; r = rn, rn = (taken < nstat ? gw + taken * nwarps : __shfl_sync(kFull, ticket, 0) + dynbase), taken++,
+                  parity ^= 1u) {
     cp_wait<0>();
     __syncwarp();
-    prefetch_replica(r + nwarps, parity ^ 1u);
+    prefetch_replica(rn, parity ^ 1u);
+    if (taken >= nstat && lane == 0) ticket = atomicAdd(A.count + 4, 1u);
     const unsigned long long* sh = reinterpret_cast<const unsigned long long*>(X.hdr[parity]);
     unsigned long long* h64 = reinterpret_cast<unsigned long long*>(s.hdr + r);
     const unsigned long long w13 = sh[13];
