@@ -33,7 +33,7 @@ if ROOT not in sys.path:
 
 from paper_2606_18431_b200 import workloads as W  # noqa: E402
 
-KERNELS_PER_ROUND = 2                # ub::k_stream + the L launch of ub::k_step (every config-5 replica is stream-eligible)
+KERNELS_PER_ROUND = 4                # a round = two halves on two streams, each ub::k_stream + the L launch of ub::k_step
 TRAFFIC_BYTES_PER_LAUNCH = 483.7e6   # dram read+write bytes of one ub::k_stream launch, profiles/r01c_stream.md (ncu --set full)
 ALG_BYTES_PER_REQUEST_STEP = 40      # read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
 METRIC = "request-steps scheduled/sec"
@@ -256,9 +256,10 @@ def main():
                          "alg_bytes_per_request_step": ALG_BYTES_PER_REQUEST_STEP,
                          "request_steps_per_launch": (rs2 - rs1) / max(1, rounds),
                          "avg_launch_ms": ms / max(1, rounds),
-                         "note": "avg_launch_ms = timed region / scheduler rounds: one k_stream launch plus the four "
-                                 "(empty in this config) team-kernel launches, so the kernel alone is slightly faster; "
-                                 "traffic = dram read+write bytes of one k_stream launch from profiles/ (ncu --set full)"},
+                         "note": "a round = every live replica advanced one iteration = two overlapping k_stream launches "
+                                 "(one half of the replicas each, on two streams) + two (empty here) team-kernel launches; "
+                                 "avg_launch_ms, request_steps_per_launch and traffic are per round; traffic = dram "
+                                 "read+write bytes of the round's k_stream launches from profiles/ (ncu --set full)"},
             "e2e": {"value": rs_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
                     "note": "one job: ub_create + ub_load_trace from pinned host + ub_set_replicas + spin-up + warm-up + timed steps + 2x ub_stats D2H; all request-steps / wall"},
             "gpu_launches": launches, "clocks": clocks,

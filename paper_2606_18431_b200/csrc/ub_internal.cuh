@@ -80,7 +80,8 @@ struct SimDev {                 // kernel argument (by value)
 };
 
 // kernels (ub_step.cu, ub_aux.cu)
-void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, cudaStream_t st);
+void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
+                 cudaStream_t st);
 void launch_stream(const struct StepArgs& A, cudaStream_t st);    // ub_stream.cu
 size_t step_smem_bytes(uint32_t Q);
 int  step_configure(uint32_t Q);

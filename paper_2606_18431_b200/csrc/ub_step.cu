@@ -697,16 +697,17 @@ int step_configure(uint32_t) {
 // One scheduler round (`iters` iterations of every live replica): the streaming kernel (ub_stream.cu) visits every
 // replica and queues what it does not handle (SRPT / LAS keys, test-only modes, re-key bursts) for the team kernels:
 // L list, M list, S list, then the overflow list.
-void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, cudaStream_t st) {
+void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
+                 cudaStream_t st) {
   StepArgs A;
-  A.s = s; A.list = list; A.count = count; A.iters = iters;
+  A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
   if (s.all_stream) A.thrS = A.thrM = 0;                                        // (windows are never empty when queued)
   cudaMemsetAsync(count, 0, 5 * sizeof(uint32_t), st);                          // this round's lists and ticket counter
   launch_stream(A, st);
-  const uint32_t R = s.R;
+  const uint32_t R = rend - rbeg;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;
   const uint32_t nS = (R + kTeamsS - 1) / kTeamsS, gS = nS < 148u * 10 ? nS : 148u * 10;
   k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 2u, 0xFFFFFFFFu);

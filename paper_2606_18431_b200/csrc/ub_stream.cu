@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 
   // header, parameters, dirty list and the first two chunks of replica rr -> stage `par` (one cp.async group)
   auto prefetch_replica = [&](const uint32_t rr, const uint32_t par) {
-    if (rr < s.R) {
+    if (rr < A.rend) {
       if (lane < 10) cp16(&X.hdr[par][lane], reinterpret_cast<const uint4*>(s.hdr + rr) + lane);
       else if (lane < 12) cp16(&X.par[par][lane - 10], reinterpret_cast<const uint4*>(s.par + rr) + (lane - 10));
       else if (lane < 16)
@@ -104,15 +104,15 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   // Work distribution: windows differ by two orders of magnitude.  A warp takes its first `nstat` replicas by static
   // striding (3/4 of an even share); the rest are handed out dynamically: each is the next value of a global ticket
   // counter (count[4], zeroed per round), requested one replica ahead so that the atomic's latency is never waited for.
-  const uint32_t gw = blockIdx.x * kSWarps + wib;
-  const uint32_t share = (s.R / nwarps) * 3u / 4u;
+  const uint32_t gw = A.rbeg + blockIdx.x * kSWarps + wib;
+  const uint32_t share = ((A.rend - A.rbeg) / nwarps) * 3u / 4u;
   const uint32_t nstat = share > 2u ? share : 2u;
-  const uint32_t dynbase = nstat * nwarps;
+  const uint32_t dynbase = A.rbeg + nstat * nwarps;
   uint32_t r = gw, rn = gw + nwarps;
   uint32_t taken = 2, ticket = 0;
   uint32_t parity = 0;
   prefetch_replica(r, 0);
-  for (; r < s.R; r = rn, rn = (taken < nstat ? gw + taken * nwarps : __shfl_sync(kFull, ticket, 0) + dynbase), taken++,
+  for (; r < A.rend; r = rn, rn = (taken < nstat ? gw + taken * nwarps : __shfl_sync(kFull, ticket, 0) + dynbase), taken++,
                   parity ^= 1u) {
     cp_wait<0>();
     __syncwarp();
@@ -651,7 +651,7 @@ void launch_stream(const StepArgs& A, cudaStream_t st) {
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  const uint32_t need = (A.s.R + kSWarps - 1) / kSWarps;
+  const uint32_t need = (A.rend - A.rbeg + kSWarps - 1) / kSWarps;
   uint32_t grid = (uint32_t)(sms * ctas_per_sm);
   if (grid > need) grid = need;
   k_stream<<<grid, 32 * kSWarps, 0, st>>>(A);

@@ -261,3 +261,36 @@ def test_configs_sampled_full_run(gpu, oracle_mod, cfg_id, kw, picks):
     _assert_same(g, o, wl.name)
     _assert_hist_same(g, o, range(wl.R))
     assert all(s["done"] == 1 for s in g.stats())
+
+
+# ------------------------------------------------------------------------------------------ config 5 at full size
+
+def test_config5_full_size_sampled(gpu, oracle_mod):
+    """BASELINE.json configs[4] at its full size (65536 replicas x 8192 requests) in the launch configuration
+    bench.py times (one iteration per launch, rounds split over two streams): run to completion, then the schedule
+    digest, the counters and the integer / fp64 percentiles of sampled replicas against the oracle, which computes
+    those replicas one by one (a replica's schedule does not depend on the batch around it, pin P14)."""
+    R, N = 65536, 8192
+    wl = W.config5(n_seeds=R, n_requests=N)
+    import os
+    tr = wl.traces(workers=max(1, min(32, os.cpu_count() or 1)))
+    g = gpu.Sim(wl.sim, wl.replicas, tr, iters_per_launch=1)
+    g.run()
+    dg = g.digest()
+    raw = g.stats_raw()
+    picks = [0, 1, 4095, 8191, 16384, 32767, 32768, 32769, 40000, 50001, 65534, 65535]
+    sub = wl.select(picks)
+    o = oracle_mod.OracleSim(sub.sim, sub.replicas, tuple(x[picks] for x in tr))
+    o.run()
+    do, so = o.digest(), o.stats()
+    for j, r in enumerate(picks):
+        assert dg[r] == do[j], f"replica {r}: schedule digest"
+        a = gpu._stats_to_dict(raw[r])
+        for k in INT_STATS:
+            assert a[k] == so[j][k], f"replica {r} stat {k}: gpu {a[k]} oracle {so[j][k]}"
+        for k in F64_STATS:
+            av, bv = np.atleast_1d(a[k]).astype(float), np.atleast_1d(so[j][k]).astype(float)
+            assert np.all(np.abs(av - bv) <= REL_TOL * np.maximum(1e-300, np.abs(bv))), f"replica {r} {k}"
+    done = np.array([raw[r].done for r in range(0, R, 97)])
+    assert done.all()
+    g.close(); o.close()
