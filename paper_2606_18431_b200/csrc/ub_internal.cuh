@@ -55,6 +55,7 @@ struct __align__(16) RepPar {   // per-replica parameters, read-only on the devi
   uint8_t  policy, guard, signal_mode, quant_mode;
   uint32_t pad[2];
 };
+constexpr uint32_t kMaxSplit = 4;     // parts (streams) a scheduler round may be issued as
 constexpr uint32_t kWindowPad = 64;   // records allocated behind the last window (speculative chunk reads)
 
 struct SimDev {                 // kernel argument (by value)

@@ -228,7 +228,10 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       // newcomer was blocked on KV), 2 = stopped; carryW / carryC = tokens / KV blocks claimed so far; crank = rank of
       // the next request in the merged order (mode 0); carryN = requests admitted so far (mode 1).
       uint32_t mode = 0, carryW = 0, carryC = 0, carryN = 0, crank = 0;
-      uint32_t pf = 0, dec = 0, kres = 0, evl = 0, evu = 0, emit = 0, same = 0, swb = 0, swc = 0;   // per-lane sums
+      // per-lane sums: de = decode sequences | tokens emitted << 16; ps = prefill tokens | same-gap emissions << 16
+      // (each field < 2^16: M, Q <= 2048, T <= 65535); swap-ins (rare) are summed in shared memory
+      uint32_t de = 0, ps = 0, kres = 0, evl = 0, evu = 0;
+      if (lane == 0) X.skb[0].w = 0u, X.skb[1].w = 0u;                // (the spare words of the parking area)
       uint32_t outpos = 0, nev = 0, ndnew = 0, n_done = 0;
       uint32_t dptr = 0;                                              // next parked request to merge
 
@@ -298,8 +301,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         // ---- batch totals (M9) and events (M12)
         const bool adm = want != 0u;
         const bool isdec = adm && w1.d >= 1u && rem == 1u;            // decode sequence vs prefill tokens
-        dec += isdec ? 1u : 0u;
-        pf += isdec ? 0u : want;
+        de += isdec ? 1u : 0u;
+        ps += isdec ? 0u : want;
         {
           const uint32_t m32 = ((w1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu);
           const uint64_t h = (uint64_t)m32 * (uint64_t)(2u * want + 1u);
@@ -310,7 +313,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         if (__any_sync(kFull, swp)) {                                 // swap-in on admission (rare)
           if (swp) {
             const uint32_t blocks = (w1.cached + blk_m1) >> blk_sh;
-            swb += blocks; swc++;
+            atomicAdd(&X.skb[0].w, blocks); atomicAdd(&X.skb[1].w, 1u);
             ev_add(evl, evu, EV_SWAPIN, w1.id, blocks);
           }
         }
@@ -323,8 +326,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const bool emitted = adm && cached2 == sig;                   // KV caught up => one token out (M2)
         const bool ep_old = (of & F_EMITPREV) != 0;
         const uint32_t d2 = d_old + (emitted ? 1u : 0u);
-        emit += emitted ? 1u : 0u;
-        same += (emitted && d_old != 0u && ep_old) ? 1u : 0u;         // gap == this iteration's cost
+        de += emitted ? 0x10000u : 0u;
+        ps += (emitted && d_old != 0u && ep_old) ? 0x10000u : 0u;     // gap == this iteration's cost
         const bool gone = emitted && d2 == w0.D;                      // complete: KV freed at once
         uint32_t nf = of & (F_RESIDENT | F_SWAPPED);
         if (adm) nf = F_RESIDENT | F_ADMITNOW;
@@ -436,7 +439,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
                        make_int4((int)r1.id, (int)(r1.d + 1u), (int)(r1.cached + 1u), (int)fl));
                 const uint64_t h = (uint64_t)(((r1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu)) * 3ull;
                 evl += (uint32_t)h; evu += (uint32_t)(h >> 32);
-                dec++; emit++; same++;
+                de += 0x10001u; ps += 0x10000u;
               }
               crank += nv; carryW += nv; carryC += totf; outpos += nv;
               continue;
@@ -478,18 +481,17 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       __syncwarp();
 
       // ---------------- batch totals, victim select, cost
-      pf = __reduce_add_sync(kFull, pf);
-      const uint32_t de = __reduce_add_sync(kFull, dec | (emit << 16));
-      dec = de & 0xFFFFu; emit = de >> 16;
-      same = __reduce_add_sync(kFull, same);
+      de = __reduce_add_sync(kFull, de);
+      ps = __reduce_add_sync(kFull, ps);
+      const uint32_t dec = de & 0xFFFFu, emit = de >> 16, pf = ps & 0xFFFFu, same = ps >> 16;
       kres = __reduce_add_sync(kFull, kres);
       const unsigned long long w14 = reinterpret_cast<const unsigned long long*>(X.hdr[parity])[14];
       uint32_t swap_used = (uint32_t)w14;
       const uint32_t peak = (uint32_t)(w14 >> 32);
       uint32_t swin_blocks = 0, swin_cnt = 0;
-      if (__any_sync(kFull, swc != 0u)) {
-        swin_blocks = __reduce_add_sync(kFull, swb);
-        swin_cnt = __reduce_add_sync(kFull, swc);
+      if (X.skb[1].w) {
+        swin_blocks = X.skb[0].w;
+        swin_cnt = X.skb[1].w;
         swap_used -= swin_blocks;
       }
       const uint32_t C = carryC;
