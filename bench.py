@@ -33,6 +33,7 @@ if ROOT not in sys.path:
 
 from paper_2606_18431_b200 import workloads as W  # noqa: E402
 
+RESIDENT_IPL = 16
 KERNELS_PER_ROUND = 4                # a round = two halves on two streams, each ub::k_stream + the L launch of ub::k_step
 TRAFFIC_BYTES_PER_LAUNCH = 483.7e6   # dram read+write bytes of one ub::k_stream launch, profiles/r01c_stream.md (ncu --set full)
 ALG_BYTES_PER_REQUEST_STEP = 40      # read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
@@ -46,7 +47,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--iters", type=int, default=64, help="scheduler iterations per step")
+    ap.add_argument("--iters", type=int, default=128, help="scheduler iterations per step")
     ap.add_argument("--spinup", type=int, default=65536, help="untimed iterations before the warm-up")
     ap.add_argument("--replicas", type=int, default=65536, help="replicas per GPU (config5: 65536)")
     ap.add_argument("--requests", type=int, default=8192)
@@ -226,6 +227,22 @@ def main():
 
     st2 = stats_table()
     t_e2e = time.perf_counter() - t_e2e0
+
+    # resident-state mode, reported separately: 16 iterations per launch, a warp advances its
+    # replica 16 iterations in a row and the window is re-read from L2; same schedule, fewer HBM bytes
+    B.ub_set_iters_per_launch(h, RESIDENT_IPL)
+    B.ub_step(h, args.iters)
+    st3 = stats_table()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    for _ in range(args.steps):
+        B.ub_step(h, args.iters)
+    f1.record()
+    torch.cuda.synchronize()
+    ms_res = f0.elapsed_time(f1)
+    st4 = stats_table()
+    rs_res = int(st4[:, COL["request_steps"]].sum()) - int(st3[:, COL["request_steps"]].sum())
+    B.ub_set_iters_per_launch(h, args.iters_per_launch)
     rs2 = int(st2[:, COL["request_steps"]].sum())
     d2h_bytes = R * (B.C.sizeof(B.UbReplicaStats))
     ttlt_p99_us = st2[:, 14 + 3 + 2][st2[:, COL["n_completed"]] > 0]          # ttlt_us[2]
@@ -262,6 +279,9 @@ def main():
                                  "read+write bytes of the round's k_stream launches from profiles/ (ncu --set full)"},
             "e2e": {"value": rs_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
                     "note": "one job: ub_create + ub_load_trace from pinned host + ub_set_replicas + spin-up + warm-up + timed steps + 2x ub_stats D2H; all request-steps / wall"},
+            "resident": {"value": rs_res / (ms_res * 1e-3) * world, "unit": UNIT, "iters_per_launch": RESIDENT_IPL,
+                         "note": "same K steps with 16 iterations per kernel launch (window re-read from L2, not HBM); "
+                                 "per-rank value x ranks; not the roofline path"},
             "gpu_launches": launches, "clocks": clocks,
         }
         if not args.no_cpu_baseline:

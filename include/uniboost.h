@@ -153,6 +153,11 @@ int  ub_debug_get_state(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t*
  * the borrowed stream: total milliseconds and launch count.  Synchronises. */
 int  ub_last_step_timing(ub_sim*, float* kernel_ms, uint32_t* launches);
 
+/* Changes ub_config::iters_per_launch for the following ub_step / ub_run calls (0 is read as 1).  The schedule does
+ * not depend on it (pin P14): with more than one iteration per launch a warp advances its replica several iterations
+ * in a row, so the window is re-read from L2 instead of HBM.  Host call, does not synchronise. */
+int  ub_set_iters_per_launch(ub_sim*, uint32_t iters_per_launch);
+
 const char* ub_strerror(int code);
 
 #ifdef __cplusplus

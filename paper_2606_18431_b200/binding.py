@@ -51,7 +51,7 @@ class UbReplicaStats(C.Structure):
 #: every symbol include/uniboost.h declares
 EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_step", "ub_run", "ub_stats",
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
-           "ub_last_step_timing", "ub_strerror")
+           "ub_last_step_timing", "ub_set_iters_per_launch", "ub_strerror")
 
 _lib = None
 
@@ -79,6 +79,7 @@ def lib():
         L.ub_tbt_hist.argtypes = [vp, U32, vp]
         L.ub_debug_get_state.argtypes = [vp, U32, P(U32), vp, vp, vp, vp, P(I64)]
         L.ub_last_step_timing.argtypes = [vp, P(C.c_float), P(U32)]
+        L.ub_set_iters_per_launch.argtypes = [vp, U32]
         L.ub_strerror.argtypes = [C.c_int]; L.ub_strerror.restype = C.c_char_p
         _lib = L
     return _lib
@@ -120,6 +121,10 @@ def ub_load_trace(h, arrival_us, prompt_tok, decode_tok, n_req, ptrs_on_device=F
 
 def ub_set_replicas(h, reps):
     return _chk(lib().ub_set_replicas(h, reps))
+
+
+def ub_set_iters_per_launch(h, iters_per_launch):
+    _chk(lib().ub_set_iters_per_launch(h, int(iters_per_launch)))
 
 
 def ub_step(h, n_iters, want_live=False):

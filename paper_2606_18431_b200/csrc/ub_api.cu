@@ -394,6 +394,12 @@ int ub_last_step_timing(ub_sim* s, float* ms, uint32_t* launches) {
   return UB_OK;
 }
 
+int ub_set_iters_per_launch(ub_sim* s, uint32_t ipl) {
+  if (!s) return UB_EINVAL;
+  s->cfg.iters_per_launch = ipl ? ipl : 1;
+  return UB_OK;
+}
+
 int ub_stats(ub_sim* s, ub_replica_stats* out) {
   if (!s || !out) return UB_EINVAL;
   if (!s->have_reps) return UB_ESTATE;
