@@ -263,34 +263,46 @@ def test_configs_sampled_full_run(gpu, oracle_mod, cfg_id, kw, picks):
     assert all(s["done"] == 1 for s in g.stats())
 
 
-# ------------------------------------------------------------------------------------------ config 5 at full size
+# ------------------------------------------------------------------------------------------ full sizes, sampled replicas
 
-def test_config5_full_size_sampled(gpu, oracle_mod):
-    """BASELINE.json configs[4] at its full size (65536 replicas x 8192 requests) in the launch configuration
-    bench.py times (one iteration per launch, rounds split over two streams): run to completion, then the schedule
-    digest, the counters and the integer / fp64 percentiles of sampled replicas against the oracle, which computes
-    those replicas one by one (a replica's schedule does not depend on the batch around it, pin P14)."""
-    R, N = 65536, 8192
-    wl = W.config5(n_seeds=R, n_requests=N)
+def _full_size_sampled(gpu, oracle_mod, wl, picks):
+    """Run the whole workload on the GPU in bench.py's launch configuration (one iteration per launch), then compare
+    the schedule digest, the counters and the integer / fp64 percentiles of the sampled replicas with the oracle,
+    which computes those replicas one by one (a replica's schedule does not depend on the batch around it, P14)."""
     import os
     tr = wl.traces(workers=max(1, min(32, os.cpu_count() or 1)))
     g = gpu.Sim(wl.sim, wl.replicas, tr, iters_per_launch=1)
     g.run()
     dg = g.digest()
     raw = g.stats_raw()
-    picks = [0, 1, 4095, 8191, 16384, 32767, 32768, 32769, 40000, 50001, 65534, 65535]
     sub = wl.select(picks)
-    o = oracle_mod.OracleSim(sub.sim, sub.replicas, tuple(x[picks] for x in tr))
+    tid = wl.replicas["trace_id"][np.asarray(picks)]
+    used = np.unique(tid)
+    o = oracle_mod.OracleSim(sub.sim, sub.replicas, tuple(x[used] for x in tr))
     o.run()
     do, so = o.digest(), o.stats()
     for j, r in enumerate(picks):
-        assert dg[r] == do[j], f"replica {r}: schedule digest"
+        assert dg[r] == do[j], f"{wl.name} replica {r}: schedule digest"
         a = gpu._stats_to_dict(raw[r])
         for k in INT_STATS:
-            assert a[k] == so[j][k], f"replica {r} stat {k}: gpu {a[k]} oracle {so[j][k]}"
+            assert a[k] == so[j][k], f"{wl.name} replica {r} stat {k}: gpu {a[k]} oracle {so[j][k]}"
         for k in F64_STATS:
             av, bv = np.atleast_1d(a[k]).astype(float), np.atleast_1d(so[j][k]).astype(float)
-            assert np.all(np.abs(av - bv) <= REL_TOL * np.maximum(1e-300, np.abs(bv))), f"replica {r} {k}"
-    done = np.array([raw[r].done for r in range(0, R, 97)])
-    assert done.all()
+            assert np.all(np.abs(av - bv) <= REL_TOL * np.maximum(1e-300, np.abs(bv))), f"{wl.name} replica {r} {k}"
+    assert all(raw[r].done for r in range(0, wl.R, 97))
     g.close(); o.close()
+
+
+@pytest.mark.parametrize("cfg_id,picks", [
+    (2, [0, 1, 2, 1535, 1536, 1537, 3069, 3070, 3071]),            # 1024 seeds x {FCFS, SRPT, BOOST}
+    (3, [0, 1, 2047, 2048, 3000, 4095]),                            # 4096 replicas, MMPP-2, swap-vs-recompute
+    (4, [0, 7, 15, 8191, 8192, 8200, 16368, 16383]),                # 1024 seeds x 16 gamma
+])
+def test_configs_full_size_sampled(gpu, oracle_mod, cfg_id, picks):
+    _full_size_sampled(gpu, oracle_mod, W.by_id(cfg_id), picks)
+
+
+def test_config5_full_size_sampled(gpu, oracle_mod):
+    """BASELINE.json configs[4] at its full size (65536 replicas x 8192 requests; rounds split over two streams)."""
+    _full_size_sampled(gpu, oracle_mod, W.config5(n_seeds=65536, n_requests=8192),
+                       [0, 1, 4095, 8191, 16384, 32767, 32768, 32769, 40000, 50001, 65534, 65535])
