@@ -44,6 +44,11 @@ class OrcStats(C.Structure):
         ("tokens_per_s", C.c_double)]
 
 
+class OrcGammaAda(C.Structure):
+    _fields_ = [("window", I64), ("min_samples", I64), ("beta_shift", I64), ("levels", I64),
+                ("gamma_min", C.c_double), ("gamma_max", C.c_double), ("eps_us", I64)]
+
+
 class OrcStepEntry(C.Structure):
     _fields_ = [(n, I64) for n in ("id", "klass", "key", "bin", "resident_before", "want", "evict",
                                    "cached_after", "d_after", "resident_after")]
@@ -80,6 +85,10 @@ def lib():
         L.orc_percentile_nearest_rank.argtypes = [C.c_void_p, I64, I64]; L.orc_percentile_nearest_rank.restype = I64
         L.orc_tbt_bin.argtypes = [I64]; L.orc_tbt_bin.restype = I64
         L.orc_tbt_edge.argtypes = [I64]; L.orc_tbt_edge.restype = I64
+        L.orc_set_gamma_ada.argtypes = [C.c_void_p, P(OrcGammaAda), C.c_void_p]
+        L.orc_gamma_state.argtypes = [C.c_void_p, I64, P(I64), P(I64), P(I64)]
+        L.orc_gamma_grid.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_gamma_hat_u.argtypes = [I64, I64, I64]; L.orc_gamma_hat_u.restype = I64
         L.orc_strerror.argtypes = [C.c_int]; L.orc_strerror.restype = C.c_char_p
         _lib = L
     return _lib
@@ -106,6 +115,10 @@ def quant_bin(sig, k):
 
 def boost_us(gamma, w_tokens, tok_us):
     return int(lib().orc_boost_us(float(gamma), int(w_tokens), int(tok_us)))
+
+
+def gamma_hat_u(t95_us, t99_us, eps_us):
+    return int(lib().orc_gamma_hat_u(int(t95_us), int(t99_us), int(eps_us)))
 
 
 def percentile_nearest_rank(sorted_vals, p):
@@ -152,6 +165,24 @@ class OracleSim:
             reps[r].gamma = float(replicas["gamma"][r])
         _chk(L.orc_set_replicas(h, reps))
         self.R, self.N, self.Q = R, int(sim["max_requests"]), int(sim["queue_cap"])
+
+    def set_gamma_ada(self, ada: dict, adaptive):
+        """gamma-Ada (M13): ada = dict(window, min_samples, beta_shift, levels, gamma_min, gamma_max, eps_us)."""
+        g = OrcGammaAda(**{n: (float(ada[n]) if n.startswith("gamma") else int(ada[n])) for n, _ in OrcGammaAda._fields_})
+        ad = np.ascontiguousarray(adaptive, np.uint8)
+        assert ad.shape == (self.R,)
+        _chk(lib().orc_set_gamma_ada(self._h, C.byref(g), ad.ctypes.data))
+        self._levels = int(ada["levels"])
+
+    def gamma_state(self, r=0):
+        g, l, n = I64(0), I64(0), I64(0)
+        _chk(lib().orc_gamma_state(self._h, int(r), C.byref(g), C.byref(l), C.byref(n)))
+        return g.value, l.value, n.value
+
+    def gamma_grid(self):
+        out = np.zeros(self._levels, np.int64)
+        _chk(lib().orc_gamma_grid(self._h, out.ctypes.data))
+        return out
 
     @classmethod
     def from_workload(cls, wl, workers: int = 1):

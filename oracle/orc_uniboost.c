@@ -41,6 +41,11 @@ typedef struct {
   int64_t iterations, request_steps, n_completed, evict_recompute, evict_swap, swapins;
   int64_t tokens_lost, tokens_emitted, prefill_tokens, decode_seqs, peak_active;
   int64_t sum_ttft, sum_ttlt, sum_tbt_num, sum_tbt_den;
+  /* gamma-Ada (M13) */
+  int32_t ada;
+  int64_t* ring;       /* [window] E2E latencies, slot = completion number mod window */
+  int64_t* lut_levels; /* [levels][LUT_CAP_GEOM] */
+  int64_t gamma_u, level, n_updates, seen;
 } orc_rep;
 
 struct orc_sim {
@@ -48,6 +53,8 @@ struct orc_sim {
   int64_t* arrival; int32_t* prompt; int32_t* decode; uint32_t* n_req;
   int have_trace, have_reps;
   orc_rep* rep;
+  orc_gamma_ada ada; int have_ada;
+  int64_t* grid_u;     /* [levels] */
 };
 
 /* ---------- small closed-form helpers ---------- */
@@ -153,9 +160,12 @@ int orc_create(const orc_config* c, orc_sim** out) {
 static void free_reps(orc_sim* s) {
   if (!s->rep) return;
   for (int64_t r = 0; r < s->cfg.n_replicas; r++) {
-    free(s->rep[r].req); free(s->rep[r].active); free(s->rep[r].lut); free(s->rep[r].hist);
+    free(s->rep[r].req); free(s->rep[r].active); free(s->rep[r].hist);
+    if (!s->rep[r].ada) free(s->rep[r].lut);          /* (an adaptive replica's lut points into lut_levels) */
+    free(s->rep[r].ring); free(s->rep[r].lut_levels);
   }
   free(s->rep); s->rep = NULL; s->have_reps = 0;
+  free(s->grid_u); s->grid_u = NULL; s->have_ada = 0;
 }
 
 void orc_destroy(orc_sim* s) {
@@ -245,6 +255,110 @@ int orc_set_replicas(orc_sim* s, const orc_replica* reps) {
   return ORC_OK;
 }
 
+
+/* ---------- gamma-Ada (M13) ---------- */
+
+#define LN5_E12 1609437912434LL   /* floor(ln(5) * 1e12) */
+
+/* Eq. 9 with F(t95) = 0.05, F(t99) = 0.01: gamma_hat = ln 5 / (t99 - t95), times in seconds;
+ * in micro units with times in microseconds: hat_u = ln5 * 1e12 / max(t99 - t95, eps). */
+int64_t orc_gamma_hat_u(int64_t t95_us, int64_t t99_us, int64_t eps_us) {
+  int64_t delta = t99_us - t95_us;
+  if (delta < eps_us) delta = eps_us;
+  return LN5_E12 / delta;
+}
+
+static int i64_cmp_(const void* a, const void* b) {
+  int64_t x = *(const int64_t*)a, y = *(const int64_t*)b;
+  return (x > y) - (x < y);
+}
+
+static int64_t level_of(const orc_sim* s, int64_t gamma_u) {
+  int64_t j = 0;
+  while (j + 1 < s->ada.levels && s->grid_u[j + 1] <= gamma_u) j++;
+  return j;
+}
+
+/* UPDATEGAMMA, step by step */
+static int update_gamma(orc_sim* s, orc_rep* x) {
+  const orc_gamma_ada* g = &s->ada;
+  if (x->n_completed == x->seen || x->n_completed < g->min_samples) return 0;
+  int64_t m = x->n_completed < g->window ? x->n_completed : g->window;
+  int64_t* L = (int64_t*)malloc(sizeof(int64_t) * (size_t)m);
+  if (!L) return ORC_ENOMEM;
+  memcpy(L, x->ring, sizeof(int64_t) * (size_t)m);      /* slots 0..m-1 hold the last m samples */
+  qsort(L, (size_t)m, sizeof(int64_t), i64_cmp_);
+  int64_t x95 = orc_percentile_nearest_rank(L, m, 95), x99 = orc_percentile_nearest_rank(L, m, 99);
+  free(L);
+  int64_t hat = orc_gamma_hat_u(x95, x99, g->eps_us);
+  x->gamma_u += (hat - x->gamma_u) / ((int64_t)1 << g->beta_shift);          /* (1-beta) gamma + beta gamma_hat */
+  if (x->gamma_u < s->grid_u[0]) x->gamma_u = s->grid_u[0];                   /* clip */
+  if (x->gamma_u > s->grid_u[g->levels - 1]) x->gamma_u = s->grid_u[g->levels - 1];
+  x->level = level_of(s, x->gamma_u);
+  x->lut = x->lut_levels + x->level * LUT_CAP_GEOM;
+  x->seen = x->n_completed;
+  x->n_updates++;
+  return 0;
+}
+
+int orc_set_gamma_ada(orc_sim* s, const orc_gamma_ada* g, const uint8_t* adaptive) {
+  if (!s || !g || !adaptive) return ORC_EINVAL;
+  if (!s->have_reps) return ORC_ESTATE;
+  if (g->window < s->cfg.max_batch || g->window > 1024 || g->min_samples < 2 || g->beta_shift < 0 ||
+      g->beta_shift > 16 || g->levels < 2 || g->levels > 64 || !(g->gamma_min > 0.0) ||
+      !(g->gamma_max > g->gamma_min) || g->gamma_max > 1e6 || g->eps_us < 1)
+    return ORC_EINVAL;
+  for (int64_t r = 0; r < s->cfg.n_replicas; r++) {
+    const orc_rep* x = &s->rep[r];
+    if (adaptive[r] && (x->par.policy != ORC_BOOST || x->par.quant_mode != ORC_Q_GEOMETRIC || isinf(x->par.gamma)))
+      return ORC_EINVAL;
+    if (x->iterations != 0 || x->ada) return ORC_ESTATE;
+  }
+  s->ada = *g; s->have_ada = 1;
+  free(s->grid_u);
+  s->grid_u = (int64_t*)calloc((size_t)g->levels, sizeof(int64_t));
+  if (!s->grid_u) return ORC_ENOMEM;
+  for (int64_t j = 0; j < g->levels; j++) {
+    double gj = g->gamma_min * pow(g->gamma_max / g->gamma_min, (double)j / (double)(g->levels - 1));
+    s->grid_u[j] = (int64_t)floor(gj * 1e6 + 0.5);
+  }
+  for (int64_t r = 0; r < s->cfg.n_replicas; r++) {
+    orc_rep* x = &s->rep[r];
+    if (!adaptive[r]) continue;
+    x->ring = (int64_t*)calloc((size_t)g->window, sizeof(int64_t));
+    x->lut_levels = (int64_t*)calloc((size_t)(g->levels * LUT_CAP_GEOM), sizeof(int64_t));
+    if (!x->ring || !x->lut_levels) return ORC_ENOMEM;
+    for (int64_t j = 0; j < g->levels; j++) {
+      double gj = g->gamma_min * pow(g->gamma_max / g->gamma_min, (double)j / (double)(g->levels - 1));
+      for (int64_t b = 0; b < LUT_CAP_GEOM; b++)
+        x->lut_levels[j * LUT_CAP_GEOM + b] = boost_fixed(gj, ldexp((double)s->cfg.bin_tokens, (int)b), s->cfg.tok_us);
+    }
+    x->gamma_u = (int64_t)floor(x->par.gamma * 1e6 + 0.5);
+    if (x->gamma_u < s->grid_u[0]) x->gamma_u = s->grid_u[0];
+    if (x->gamma_u > s->grid_u[g->levels - 1]) x->gamma_u = s->grid_u[g->levels - 1];
+    x->level = level_of(s, x->gamma_u);
+    free(x->lut);
+    x->lut = x->lut_levels + x->level * LUT_CAP_GEOM; x->nb = LUT_CAP_GEOM;
+    x->ada = 1;
+  }
+  return ORC_OK;
+}
+
+int orc_gamma_state(orc_sim* s, int64_t r, int64_t* gamma_u, int64_t* level, int64_t* n_updates) {
+  if (!s || !s->have_reps || r < 0 || r >= s->cfg.n_replicas) return ORC_EINVAL;
+  const orc_rep* x = &s->rep[r];
+  if (gamma_u) *gamma_u = x->ada ? x->gamma_u : 0;
+  if (level) *level = x->ada ? x->level : -1;
+  if (n_updates) *n_updates = x->n_updates;
+  return ORC_OK;
+}
+
+int orc_gamma_grid(orc_sim* s, int64_t* grid_u) {
+  if (!s || !grid_u || !s->have_ada) return ORC_EINVAL;
+  memcpy(grid_u, s->grid_u, sizeof(int64_t) * (size_t)s->ada.levels);
+  return ORC_OK;
+}
+
 /* ---------- one scheduler iteration of one replica ---------- */
 
 typedef struct { int64_t klass, key, id, bin; int32_t resident_before; int64_t want; int32_t evict; } ent_t;
@@ -273,6 +387,8 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
     if (x->next >= nreq) return 0;            /* done: no-op */
     if (A[x->next] > x->t) x->t = A[x->next];
   }
+  /* Algorithm 1 "gamma <- UPDATEGAMMA(S)" at the top of the loop */
+  if (x->ada) { int rc = update_gamma(s, x); if (rc) return rc; }
   while (x->next < nreq && A[x->next] <= x->t && x->n_active < c->queue_cap)
     x->active[x->n_active++] = (int32_t)x->next++;
   const int64_t n = x->n_active;
@@ -387,6 +503,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
       q->t_last = t_end;
       if (q->d == Dd[id]) {
         q->completed = 1; q->resident = 0; q->cached = 0;     /* KV freed at once */
+        if (x->ada) x->ring[x->n_completed % s->ada.window] = q->t_last - A[id];   /* E2E latency sample (M13) */
         x->n_completed++;
         x->sum_ttft += q->t_first - A[id]; x->sum_ttlt += q->t_last - A[id];
         x->sum_tbt_num += q->t_last - q->t_first; x->sum_tbt_den += Dd[id] - 1;

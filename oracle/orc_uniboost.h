@@ -140,6 +140,28 @@ int  orc_digest(orc_sim*, uint64_t* digest /* [R] */);
 int  orc_boost_lut(orc_sim*, int64_t replica, int64_t* lut /* [cap] */, int64_t cap, int64_t* nb);
 int  orc_tbt_hist(orc_sim*, int64_t replica, uint32_t* hist /* [4352] */);
 /* stand-alone helpers exposed so the pins can hit them directly */
+/* gamma-Ada (rule M13 of DESIGN.md; Eq. 9 and UPDATEGAMMA), integer-only:
+ *   gamma is kept as gamma_u = gamma * 1e6 (1/s in micro units).  At the start of an executed iteration of an
+ *   adaptive replica, if a request completed since the last update and at least min_samples have completed:
+ *     L     = the last min(window, n_completed) E2E latencies (TTLT, us)
+ *     t95, t99 = nearest-rank percentiles of L (t_p of PAPER.md:225)
+ *     hat_u = floor(ln(5) * 1e12) / max(t99 - t95, eps_us)          (Eq. 9: -(ln 0.01 - ln 0.05)/(t99 - t95))
+ *     gamma_u += (hat_u - gamma_u) / 2^beta_shift  (C division, truncating);  clip to [gamma_min_u, gamma_max_u]
+ *     level = largest j with grid_u[j] <= gamma_u;  the boost table in use is the one of grid point j,
+ *   grid: gamma_j = gamma_min * (gamma_max/gamma_min)^(j/(levels-1)), grid_u[j] = floor(gamma_j*1e6 + 0.5). */
+typedef struct {
+  int64_t window;        /* W: max_batch <= W <= 1024 */
+  int64_t min_samples;   /* >= 2 */
+  int64_t beta_shift;    /* beta = 2^-beta_shift, 0..16 */
+  int64_t levels;        /* G: 2..64 */
+  double  gamma_min, gamma_max;
+  int64_t eps_us;        /* >= 1 */
+} orc_gamma_ada;
+/* after orc_set_replicas; adaptive[r] != 0 requires policy BOOST with the geometric quantiser */
+int  orc_set_gamma_ada(orc_sim*, const orc_gamma_ada* cfg, const uint8_t* adaptive /* [R] */);
+int  orc_gamma_state(orc_sim*, int64_t replica, int64_t* gamma_u, int64_t* level, int64_t* n_updates);
+int  orc_gamma_grid(orc_sim*, int64_t* grid_u /* [levels] */);
+int64_t orc_gamma_hat_u(int64_t t95_us, int64_t t99_us, int64_t eps_us);     /* Eq. 9 in fixed point */
 int64_t orc_quant_bin(int64_t sig, int64_t k);                       /* Eq. 8 exponent */
 int64_t orc_boost_us(double gamma, int64_t w_tokens, int64_t tok_us); /* Eq. 2 in fixed point */
 int64_t orc_percentile_nearest_rank(const int64_t* sorted, int64_t m, int64_t p);
