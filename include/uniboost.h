@@ -153,6 +153,34 @@ int  ub_debug_get_state(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t*
  * the borrowed stream: total milliseconds and launch count.  Synchronises. */
 int  ub_last_step_timing(ub_sim*, float* kernel_ms, uint32_t* launches);
 
+/* gamma-Ada (Eq. 9, UPDATEGAMMA PAPER.md:588-601; rule M13 of DESIGN.md),
+ * integer-only so that schedules stay bit-exact.  gamma is kept as gamma_u = gamma * 1e6.  At the start of an executed
+ * iteration of an adaptive replica, if a request completed since the last update and >= min_samples have completed:
+ *   L = the last min(window, n_completed) end-to-end latencies (us);  t95, t99 = nearest-rank percentiles of L;
+ *   hat_u = floor(ln 5 * 1e12) / max(t99 - t95, eps_us);  gamma_u += (hat_u - gamma_u) / 2^beta_shift (truncating);
+ *   clip to the grid ends;  level = largest j with grid_u[j] <= gamma_u;  the boost table of grid point j is used.
+ * Grid: gamma_j = gamma_min (gamma_max/gamma_min)^(j/(levels-1)), grid_u[j] = floor(gamma_j 1e6 + 0.5). */
+typedef struct {
+  uint32_t struct_size;
+  uint32_t window;         /* max_batch <= window <= 1024 */
+  uint32_t min_samples;    /* >= 2 */
+  uint32_t beta_shift;     /* smoothing beta = 2^-beta_shift, 0..16 */
+  uint32_t levels;         /* 2..64 */
+  uint32_t pad;
+  double   gamma_min, gamma_max;
+  int64_t  eps_us;         /* >= 1 */
+} ub_gamma_ada;
+
+/* After ub_set_replicas and before the first ub_step.  adaptive: host, [n_replicas], non-zero = the replica adapts
+ * (requires policy UB_BOOST with the geometric quantiser and a finite gamma, else UB_EINVAL); its initial gamma is its
+ * ub_replica::gamma clipped to the grid.  While adaptation is on every launch advances one iteration.  Synchronises. */
+int  ub_set_gamma_ada(ub_sim*, const ub_gamma_ada* cfg, const uint8_t* adaptive);
+/* Current gamma_u, grid level and number of updates of one replica (level = -1 for a non-adaptive one); any output
+ * nullable.  Synchronises. */
+int  ub_gamma_state(ub_sim*, uint32_t replica, int64_t* gamma_u, int32_t* level, uint64_t* n_updates);
+/* The grid (host, [levels]) as built by the library, for comparison with the oracle's. */
+int  ub_gamma_grid(ub_sim*, int64_t* grid_u);
+
 /* Changes ub_config::iters_per_launch for the following ub_step / ub_run calls (0 is read as 1).  The schedule does
  * not depend on it (pin P14): with more than one iteration per launch a warp advances its replica several iterations
  * in a row, so the window is re-read from L2 instead of HBM.  Host call, does not synchronise. */

@@ -49,9 +49,15 @@ class UbReplicaStats(C.Structure):
 
 
 #: every symbol include/uniboost.h declares
+class UbGammaAda(C.Structure):
+    _fields_ = [("struct_size", U32), ("window", U32), ("min_samples", U32), ("beta_shift", U32), ("levels", U32),
+                ("pad", U32), ("gamma_min", C.c_double), ("gamma_max", C.c_double), ("eps_us", I64)]
+
+
 EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_step", "ub_run", "ub_stats",
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
-           "ub_last_step_timing", "ub_set_iters_per_launch", "ub_strerror")
+           "ub_last_step_timing", "ub_set_iters_per_launch", "ub_set_gamma_ada", "ub_gamma_state", "ub_gamma_grid",
+           "ub_strerror")
 
 _lib = None
 
@@ -80,6 +86,9 @@ def lib():
         L.ub_debug_get_state.argtypes = [vp, U32, P(U32), vp, vp, vp, vp, P(I64)]
         L.ub_last_step_timing.argtypes = [vp, P(C.c_float), P(U32)]
         L.ub_set_iters_per_launch.argtypes = [vp, U32]
+        L.ub_set_gamma_ada.argtypes = [vp, P(UbGammaAda), vp]
+        L.ub_gamma_state.argtypes = [vp, U32, P(I64), P(C.c_int32), P(U64)]
+        L.ub_gamma_grid.argtypes = [vp, vp]
         L.ub_strerror.argtypes = [C.c_int]; L.ub_strerror.restype = C.c_char_p
         _lib = L
     return _lib
@@ -121,6 +130,29 @@ def ub_load_trace(h, arrival_us, prompt_tok, decode_tok, n_req, ptrs_on_device=F
 
 def ub_set_replicas(h, reps):
     return _chk(lib().ub_set_replicas(h, reps))
+
+
+def ub_set_gamma_ada(h, ada: dict, adaptive):
+    """ada = dict(window, min_samples, beta_shift, levels, gamma_min, gamma_max, eps_us); adaptive: [R] of 0/1."""
+    g = UbGammaAda()
+    g.struct_size = C.sizeof(UbGammaAda)
+    for k in ("window", "min_samples", "beta_shift", "levels", "eps_us"):
+        setattr(g, k, int(ada[k]))
+    g.gamma_min, g.gamma_max = float(ada["gamma_min"]), float(ada["gamma_max"])
+    ad = np.ascontiguousarray(adaptive, np.uint8)
+    _chk(lib().ub_set_gamma_ada(h, C.byref(g), ad.ctypes.data))
+
+
+def ub_gamma_state(h, r):
+    g, l, n = I64(0), C.c_int32(0), U64(0)
+    _chk(lib().ub_gamma_state(h, int(r), C.byref(g), C.byref(l), C.byref(n)))
+    return g.value, l.value, n.value
+
+
+def ub_gamma_grid(h, levels):
+    out = np.zeros(int(levels), np.int64)
+    _chk(lib().ub_gamma_grid(h, out.ctypes.data))
+    return out
 
 
 def ub_set_iters_per_launch(h, iters_per_launch):
@@ -215,6 +247,17 @@ class Sim:
 
     def run(self, max_iters=1 << 40, check=True):
         return ub_run(self._h, max_iters, check)
+
+    def set_gamma_ada(self, ada: dict, adaptive):
+        assert len(adaptive) == self.R
+        ub_set_gamma_ada(self._h, ada, adaptive)
+        self._levels = int(ada["levels"])
+
+    def gamma_state(self, r=0):
+        return ub_gamma_state(self._h, r)
+
+    def gamma_grid(self):
+        return ub_gamma_grid(self._h, self._levels)
 
     def last_step_timing(self):
         return ub_last_step_timing(self._h)

@@ -25,6 +25,8 @@ struct ub_sim {
   int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
   uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([5] = finished replicas)
+  int64_t* d_ada_ring; AdaState* d_ada_state; int64_t* d_ada_grid;   // gamma-Ada (M13), null when off
+  std::vector<int64_t> h_ada_grid;
   uint16_t* d_dlist; uint2* d_evbuf;     // dirty lists [R][kDirtyMax]; per-iteration event scratch [R][min(M,Q)]
   unsigned long long* h_word;            // pinned
   std::vector<uint32_t> h_nreq, h_maxsig;
@@ -134,6 +136,7 @@ void ub_destroy(ub_sim* s) {
   cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
   cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dlist); cudaFree(s->d_evbuf);
+  cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);
   if (s->h_word) cudaFreeHost(s->h_word);
   if (s->ev0) cudaEventDestroy(s->ev0);
   if (s->ev1) cudaEventDestroy(s->ev1);
@@ -232,6 +235,9 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
     any_exact |= (q.quant_mode == UB_Q_EXACT);
   }
   s->have_reps = false;
+  cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);        // adaptation is set per replica table
+  s->d_ada_ring = nullptr; s->d_ada_state = nullptr; s->d_ada_grid = nullptr; s->h_ada_grid.clear();
+  s->dev.ada_ring = nullptr; s->dev.ada_state = nullptr; s->dev.ada_grid = nullptr;
   if (any_exact) {
     uint32_t* d_ms = nullptr;
     int rc = dmalloc(&d_ms, c.n_traces); if (rc) return rc;
@@ -302,7 +308,8 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
 // (the caller's and internal ones, fork / join by events): replicas are independent, so while the last warps of one
 // part finish, the other parts' CTAs already fill the freed SMs.
 static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
-  const uint32_t ipl = s->cfg.iters_per_launch > 1 ? s->cfg.iters_per_launch : 1;
+  const bool ada = s->d_ada_ring != nullptr;         // UPDATEGAMMA opens every iteration: one iteration per launch
+  const uint32_t ipl = (!ada && s->cfg.iters_per_launch > 1) ? s->cfg.iters_per_launch : 1;
   const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
   const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
   uint32_t nl = 0;
@@ -314,6 +321,7 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
     const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
     for (uint32_t i = 0; i < ns; i++) {
       const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
+      if (ada) launch_gamma_ada(s->dev, rb, re, i ? s->aux[i - 1] : s->stream);
       launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, i ? s->aux[i - 1] : s->stream);
     }
     n_iters -= k; nl++;
@@ -391,6 +399,98 @@ int ub_last_step_timing(ub_sim* s, float* ms, uint32_t* launches) {
   }
   if (ms) *ms = s->last_ms;
   if (launches) *launches = s->last_launches;
+  return UB_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- gamma-Ada (M13)
+// Grid and per-level boost tables are built here on the host in fp64 (as M4), independently of the oracle.
+static double ada_grid_gamma(const ub_gamma_ada* g, uint32_t j) {
+  return g->gamma_min * pow(g->gamma_max / g->gamma_min, (double)j / (double)(g->levels - 1));
+}
+
+int ub_set_gamma_ada(ub_sim* s, const ub_gamma_ada* g, const uint8_t* adaptive) {
+  if (!s || !g || !adaptive) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (s->d_ada_ring) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const ub_config& c = s->cfg;
+  if (g->struct_size != sizeof(ub_gamma_ada) || g->window < c.max_batch || g->window > 1024 || g->min_samples < 2 ||
+      g->beta_shift > 16 || g->levels < 2 || g->levels > 64 || !(g->gamma_min > 0.0) ||
+      !(g->gamma_max > g->gamma_min) || g->gamma_max > 1e6 || g->eps_us < 1)
+    return UB_EINVAL;
+  const size_t R = c.n_replicas;
+  for (size_t r = 0; r < R; r++)
+    if (adaptive[r] && (s->h_reps[r].policy != UB_BOOST || s->h_reps[r].quant_mode != UB_Q_GEOMETRIC ||
+                        isinf(s->h_reps[r].gamma)))
+      return UB_EINVAL;
+  // a run that already started cannot switch
+  {
+    std::vector<Hdr> hd(R);
+    CK(cudaMemcpyAsync(hd.data(), s->d_hdr, R * sizeof(Hdr), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    for (size_t r = 0; r < R; r++) if (hd[r].iterations != 0) return UB_ESTATE;
+  }
+  std::vector<int64_t> grid(g->levels);
+  for (uint32_t j = 0; j < g->levels; j++) grid[j] = (int64_t)floor(ada_grid_gamma(g, j) * 1e6 + 0.5);
+  // tables of the grid levels, appended to the static ones; adaptive replicas point at them
+  const size_t base = s->h_lut.size();
+  if (base + (size_t)g->levels * 64 >= (1ull << 32)) return UB_ENOMEM;
+  for (uint32_t j = 0; j < g->levels; j++)
+    for (uint32_t b = 0; b < 64; b++)
+      s->h_lut.push_back(boost_table_entry(ada_grid_gamma(g, j), ldexp((double)c.bin_tokens, (int)b), c.tok_us));
+  std::vector<AdaState> st(R);
+  std::vector<RepPar> par(R);
+  CK(cudaMemcpy(par.data(), s->d_par, R * sizeof(RepPar), cudaMemcpyDeviceToHost));
+  for (size_t r = 0; r < R; r++) {
+    memset(&st[r], 0, sizeof(AdaState));
+    if (!adaptive[r]) continue;
+    int64_t gu = (int64_t)floor(s->h_reps[r].gamma * 1e6 + 0.5);
+    if (gu < grid[0]) gu = grid[0];
+    if (gu > grid[g->levels - 1]) gu = grid[g->levels - 1];
+    uint32_t lvl = 0;
+    while (lvl + 1 < g->levels && grid[lvl + 1] <= gu) lvl++;
+    st[r].gamma_u = gu; st[r].level = lvl; st[r].on = 1;
+    par[r].lut_off = (uint32_t)base; par[r].lut_nb = 64;
+    s->h_lut_off[r] = (uint32_t)base; s->h_lut_nb[r] = 64;
+  }
+  int rc = UB_OK;
+  cudaFree(s->d_lut); s->d_lut = nullptr;
+  if ((rc = dmalloc(&s->d_lut, s->h_lut.size())) || (rc = dmalloc(&s->d_ada_ring, R * (size_t)g->window)) ||
+      (rc = dmalloc(&s->d_ada_state, R)) || (rc = dmalloc(&s->d_ada_grid, (size_t)g->levels)))
+    return rc;
+  CK(cudaMemcpyAsync(s->d_lut, s->h_lut.data(), s->h_lut.size() * 8, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->d_par, par.data(), R * sizeof(RepPar), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->d_ada_state, st.data(), R * sizeof(AdaState), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpyAsync(s->d_ada_grid, grid.data(), grid.size() * 8, cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemsetAsync(s->d_ada_ring, 0, R * (size_t)g->window * 8, s->stream));
+  SimDev& d = s->dev;
+  d.lut = s->d_lut; d.ada_ring = s->d_ada_ring; d.ada_state = s->d_ada_state; d.ada_grid = s->d_ada_grid;
+  d.ada_W = g->window; d.ada_G = g->levels; d.ada_min = g->min_samples; d.ada_shift = g->beta_shift; d.ada_eps = g->eps_us;
+  launch_ada_init(d, s->stream);
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaGetLastError());
+  s->h_ada_grid = grid;
+  return UB_OK;
+}
+
+int ub_gamma_state(ub_sim* s, uint32_t r, int64_t* gamma_u, int32_t* level, uint64_t* n_updates) {
+  if (!s || r >= s->cfg.n_replicas) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  AdaState st; memset(&st, 0, sizeof(st));
+  if (s->d_ada_state) {
+    CK(cudaMemcpyAsync(&st, s->d_ada_state + r, sizeof(AdaState), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+  }
+  if (gamma_u) *gamma_u = st.on ? st.gamma_u : 0;
+  if (level) *level = st.on ? (int32_t)st.level : -1;
+  if (n_updates) *n_updates = st.n_updates;
+  return UB_OK;
+}
+
+int ub_gamma_grid(ub_sim* s, int64_t* grid_u) {
+  if (!s || !grid_u || s->h_ada_grid.empty()) return UB_EINVAL;
+  memcpy(grid_u, s->h_ada_grid.data(), s->h_ada_grid.size() * 8);
   return UB_OK;
 }
 

@@ -56,6 +56,66 @@ void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t
   k_reset<<<(s.R + 127) / 128, 128, 0, st>>>(s, count);
 }
 
+// ------------------------------------------------------------------ gamma-Ada (M13; Eq. 9, UPDATEGAMMA PAPER.md:588-601)
+// Launched in front of every scheduler round while adaptation is on ("gamma <- UPDATEGAMMA(S)" opens the loop of
+// Algorithm 1).  One CTA per replica; it leaves at once unless the replica adapts, is not finished, and
+// a request completed since the last update.  Then: window of the last min(W, n_completed) end-to-end latencies ->
+// shared memory, bitonic sort, nearest-rank t95 / t99, the fixed-point update, the grid level.  A level change
+// switches the boost table (Hdr::level) and re-keys every request: n_dirty is set to overflow, so this round's
+// ordering is rebuilt from scratch by the team kernel.
+constexpr int kAdaThreads = 128;
+constexpr long long kLn5e12 = 1609437912434LL;     // floor(ln 5 * 1e12)
+
+__global__ void __launch_bounds__(kAdaThreads) k_gamma_ada(SimDev s, uint32_t rbeg) {
+  __shared__ long long v[1024];
+  const uint32_t r = rbeg + blockIdx.x;
+  AdaState* st = s.ada_state + r;
+  if (!st->on) return;
+  Hdr* h = s.hdr + r;
+  const uint32_t nc = h->n_completed;
+  if ((h->n_active == 0 && h->a_next == kNever) || nc == st->seen || nc < s.ada_min) return;
+  const uint32_t m = nc < s.ada_W ? nc : s.ada_W;
+  uint32_t npad = 1; while (npad < m) npad <<= 1;
+  const int64_t* ring = s.ada_ring + (size_t)r * s.ada_W;
+  for (uint32_t i = threadIdx.x; i < npad; i += kAdaThreads) v[i] = i < m ? (long long)ring[i] : INT64_MAX;
+  __syncthreads();
+  for (uint32_t kk = 2; kk <= npad; kk <<= 1)
+    for (uint32_t j = kk >> 1; j > 0; j >>= 1) {
+      for (uint32_t i = threadIdx.x; i < npad; i += kAdaThreads) {
+        const uint32_t l = i ^ j;
+        if (l > i) {
+          const long long a = v[i], b = v[l];
+          if ((a > b) == ((i & kk) == 0)) { v[i] = b; v[l] = a; }
+        }
+      }
+      __syncthreads();
+    }
+  if (threadIdx.x == 0) {
+    uint32_t r95 = (95u * m + 99u) / 100u, r99 = (99u * m + 99u) / 100u;      // nearest rank (t_p of PAPER.md:225)
+    if (r95 < 1) r95 = 1; if (r99 < 1) r99 = 1;
+    long long delta = v[r99 - 1] - v[r95 - 1];
+    if (delta < s.ada_eps) delta = s.ada_eps;
+    const long long hat = kLn5e12 / delta;                                     // Eq. 9 in micro units
+    long long g = st->gamma_u;
+    g += (hat - g) / (1ll << s.ada_shift);                                     // (1 - beta) gamma + beta gamma_hat
+    if (g < s.ada_grid[0]) g = s.ada_grid[0];                                  // clip
+    if (g > s.ada_grid[s.ada_G - 1]) g = s.ada_grid[s.ada_G - 1];
+    uint32_t lvl = 0;
+    while (lvl + 1 < s.ada_G && s.ada_grid[lvl + 1] <= g) lvl++;
+    st->gamma_u = g; st->seen = nc; st->n_updates++;
+    if (lvl != st->level) { st->level = lvl; h->level = lvl; h->n_dirty = kDirtyMax + 1u; }
+  }
+}
+void launch_gamma_ada(const SimDev& s, uint32_t rbeg, uint32_t rend, cudaStream_t st) {
+  if (rend > rbeg) k_gamma_ada<<<rend - rbeg, kAdaThreads, 0, st>>>(s, rbeg);
+}
+
+__global__ void k_ada_init(SimDev s) {
+  const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r < s.R && s.ada_state[r].on) s.hdr[r].level = s.ada_state[r].level;
+}
+void launch_ada_init(const SimDev& s, cudaStream_t st) { k_ada_init<<<(s.R + 127) / 128, 128, 0, st>>>(s); }
+
 // ------------------------------------------------------------------ live replicas (ub_step / ub_run)
 __global__ void k_count_live(const uint32_t* count, uint32_t R, unsigned long long* live) {
   uint32_t fin = 0;

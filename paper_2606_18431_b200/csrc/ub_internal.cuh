@@ -43,7 +43,8 @@ struct __align__(16) Hdr {
   int64_t  iterations;
   uint32_t n_active, next, swap_used, peak_active;
   uint32_t n_completed, evict_recompute, evict_swap, swapins;
-  uint32_t done, todo, n_dirty, pad2;   // todo: iterations of this round still to do (hand-over between kernels)
+  uint32_t done, todo, n_dirty, level;  // todo: iterations of this round still to do (hand-over between kernels);
+                                        // level: gamma-Ada grid level (0 for a static replica), selects the boost table
 };
 static_assert(sizeof(Hdr) == 160, "Hdr is 160 bytes");
 
@@ -57,6 +58,8 @@ struct __align__(16) RepPar {   // per-replica parameters, read-only on the devi
 };
 constexpr uint32_t kMaxSplit = 4;     // parts (streams) a scheduler round may be issued as
 constexpr uint32_t kWindowPad = 64;   // records allocated behind the last window (speculative chunk reads)
+
+struct __align__(16) AdaState { int64_t gamma_u; unsigned long long n_updates; uint32_t level, seen, on, pad; };
 
 struct SimDev {                 // kernel argument (by value)
   // configuration
@@ -77,6 +80,12 @@ struct SimDev {                 // kernel argument (by value)
   uint16_t* dlist;              // [R][kDirtyMax] window positions of the re-keyed ("dirty") requests
   uint2*    evbuf;              // [R][evcap] scratch: per-request events of one iteration that wait for t_end
   uint32_t  evcap;              // min(M, Q)
+  // gamma-Ada (M13); ada_ring == nullptr when off
+  int64_t*  ada_ring;           // [R][ada_W] end-to-end latencies, slot = completion number mod ada_W
+  struct AdaState* ada_state;   // [R]
+  const int64_t* ada_grid;      // [ada_G] gamma_u thresholds
+  uint32_t  ada_W, ada_G, ada_min, ada_shift;
+  int64_t   ada_eps;
   uint32_t  all_stream;         // every replica is eligible for the streaming kernel: its rare hand-overs all go to the L team kernel
 };
 
@@ -84,6 +93,8 @@ struct SimDev {                 // kernel argument (by value)
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
                  cudaStream_t st);
 void launch_stream(const struct StepArgs& A, cudaStream_t st);    // ub_stream.cu
+void launch_gamma_ada(const SimDev& s, uint32_t rbeg, uint32_t rend, cudaStream_t st);   // ub_aux.cu
+void launch_ada_init(const SimDev& s, cudaStream_t st);
 size_t step_smem_bytes(uint32_t Q);
 int  step_configure(uint32_t Q);
 void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,

@@ -128,7 +128,9 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
   const Rec0* TR = s.TR + (size_t)par.trace_id * s.N;
   Rec0* gE0 = s.E0 + (size_t)r * s.Q;
   Rec1* gE1 = s.E1 + (size_t)r * s.Q;
-  const int64_t* lut = s.lut + par.lut_off;
+  // (a gamma-Ada replica owns one table per grid level, Hdr::level selects; 0 for a static replica)
+  const int64_t* lut = s.lut + par.lut_off + (size_t)s.hdr[r].level * 64u;
+  const uint32_t ncomp0 = s.ada_ring ? s.hdr[r].n_completed : 0u;     // (gamma-Ada runs one iteration per launch)
   int64_t* g_tfirst = s.t_first + (size_t)r * s.N;
   int64_t* g_tlast = s.t_last + (size_t)r * s.N;
   uint32_t* g_hist = s.hist + (size_t)r * kTbtBins;
@@ -582,6 +584,18 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
     }
     tm.template sum32<2>(tot2);                   // (for WARPS > 1 its barriers also publish the smem accumulators)
     if constexpr (WARPS == 1) __syncwarp();
+    if (s.ada_ring) {
+      // gamma-Ada (M13): the end-to-end latencies of this iteration's completions go to the replica's window in
+      // priority order (slot = completion number mod W)
+      uint32_t carry = ncomp0;
+#pragma unroll
+      for (int c = 0; c < E; c++) {
+        uint32_t tot;
+        const uint32_t inc = tm.scan_incl(gone[c] ? 1u : 0u, tot);
+        if (gone[c]) s.ada_ring[(size_t)r * s.ada_W + (carry + inc - 1u) % s.ada_W] = t_end - r0[c].a;
+        carry += tot;
+      }
+    }
 
     // ---------------- write back in priority order, dropping completed requests
     uint32_t n_new = 0;

@@ -76,6 +76,8 @@ __device__ __forceinline__ void score(const Rec0& q0, const Rec1& q1, uint32_t k
   bin = b;
 }
 
+// ADA: the gamma-Ada instance (per-level boost tables, latency window); the static instance carries none of it.
+template <bool ADA>
 __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   __shared__ WarpBuf wbuf[kSWarps];
   const SimDev& s = A.s;
@@ -139,7 +141,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     bool slow = !(par.policy == 0 || par.policy == 2) || par.signal_mode != 0 || par.quant_mode != 0 || blk_sh >= 32u;
     // boost table in registers: lane b holds LUT[b] (Eq. 2 in fixed point, built on the host, M4); FCFS: all 0
     int64_t lutv = 0;
-    if (isboost && !slow) lutv = __ldg(s.lut + par.lut_off + lane);   // geometric tables have 64 entries, bins < 32
+    // (a gamma-Ada replica owns one table per grid level, Hdr::level selects; 0 for a static replica)
+    if (isboost && !slow) lutv = __ldg(s.lut + par.lut_off + (ADA ? (uint32_t)(sh[18] >> 32) * 64u : 0u) + lane);   // 64 entries, bins < 32
     uint32_t it = 0;
     uint32_t wsize = n;
 
@@ -566,8 +569,15 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const uint2* gev = s.evbuf + (size_t)r * s.evcap;
         int64_t* g_tfirst = s.t_first + (size_t)r * s.N;
         int64_t* g_tlast = s.t_last + (size_t)r * s.N;
+        uint32_t cseq = ADA ? (uint32_t)reinterpret_cast<const unsigned long long*>(X.hdr[parity])[15] : 0u;   // completions so far
         for (uint32_t e0 = 0; e0 < nev; e0 += 32u) {
           const uint32_t e = e0 + (uint32_t)lane;
+          uint32_t cm = 0;
+          if constexpr (ADA) {                                        // completions of this batch, in priority order
+            uint32_t kind = 0;
+            if (e < nev) kind = __ldcg(gev + e).y;
+            cm = __ballot_sync(kFull, (kind & 4u) != 0u);
+          }
           if (e < nev) {
             const uint2 ev = __ldcg(gev + e);
             const uint32_t id = ev.x;
@@ -584,6 +594,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
               const int64_t tf = (ev.y & 1u) ? t_end : __ldcg(g_tfirst + id);
               const int4 tv = __ldg(reinterpret_cast<const int4*>(TR + id));
               const Rec0 q0 = *reinterpret_cast<const Rec0*>(&tv);
+              if constexpr (ADA)                                      // gamma-Ada: end-to-end latency sample (M13)
+                s.ada_ring[(size_t)r * s.ada_W + (cseq + __popc(cm & ltmask)) % s.ada_W] = t_end - q0.a;
               atomicAdd(h64 + 8, (unsigned long long)(tf - q0.a));
               atomicAdd(h64 + 9, (unsigned long long)(t_end - q0.a));
               atomicAdd(h64 + 10, (unsigned long long)(t_end - tf));
@@ -593,6 +605,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
               g_ne[id] = __ldcg(g_ne + id) | 0x80000000u;             // completion marker read by the stats kernel
             }
           }
+          cseq += __popc(cm);
         }
       }
       evl = __reduce_add_sync(kFull, evl);
@@ -604,6 +617,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         unsigned long long* shw = reinterpret_cast<unsigned long long*>(X.hdr[parity]);
         const uint64_t H = digest_fold(shw[1], evl, evu, t_end);
         shw[1] = H;                                                   // (kept current for a further iteration)
+        if constexpr (ADA) shw[15] += (unsigned long long)n_done | ((unsigned long long)ev_nrc << 32);
         const uint32_t pk = n > peak ? n : peak;
         shw[14] = (unsigned long long)swap_used | ((unsigned long long)pk << 32);
         if (same) atomicAdd(s.hist + (size_t)r * kTbtBins + tbt_bin(cost), same);
@@ -641,12 +655,12 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   cp_wait<0>();
 }
 
-// persistent grid: every warp strides over the replicas
-void launch_stream(const StepArgs& A, cudaStream_t st) {
+// persistent grid: every warp takes replicas until none is left
+template <bool ADA> static void launch_stream_t(const StepArgs& A, cudaStream_t st) {
   static int ctas_per_sm = 0;
   if (!ctas_per_sm) {
-    cudaFuncSetAttribute(k_stream, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream, 32 * kSWarps, 0) != cudaSuccess ||
+    cudaFuncSetAttribute(k_stream<ADA>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream<ADA>, 32 * kSWarps, 0) != cudaSuccess ||
         ctas_per_sm < 1)
       ctas_per_sm = 4;
   }
@@ -656,7 +670,10 @@ void launch_stream(const StepArgs& A, cudaStream_t st) {
   const uint32_t need = (A.rend - A.rbeg + kSWarps - 1) / kSWarps;
   uint32_t grid = (uint32_t)(sms * ctas_per_sm);
   if (grid > need) grid = need;
-  k_stream<<<grid, 32 * kSWarps, 0, st>>>(A);
+  k_stream<ADA><<<grid, 32 * kSWarps, 0, st>>>(A);
+}
+void launch_stream(const StepArgs& A, cudaStream_t st) {
+  if (A.s.ada_ring) launch_stream_t<true>(A, st); else launch_stream_t<false>(A, st);
 }
 
 }  // namespace ub
