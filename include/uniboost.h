@@ -153,6 +153,18 @@ int  ub_debug_get_state(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t*
  * the borrowed stream: total milliseconds and launch count.  Synchronises. */
 int  ub_last_step_timing(ub_sim*, float* kernel_ms, uint32_t* launches);
 
+/* Richer reductions, device-resident like ub_stats.  which: 0 = TTFT, 1 = TTLT, over the
+ * completed requests of each replica.
+ * ub_percentile_curve: nearest-rank percentiles at n (1..16) per-mille points (e.g. 500, 900, 990, 999 -- the
+ *   per-percentile curves of Fig. 6): the ceil(p m / 1000)-th smallest of the m samples (t_p of
+ *   PAPER.md:225), 0 when m = 0.  permille: host [n], each 1..1000;  out_us: host [n_replicas][n].
+ * ub_slo_attainment: for each replica and each of n (1..16) latency thresholds (microseconds; the caller forms them as
+ *   SLO scale x base latency, Fig. 8) the number of completed requests with latency <= threshold;
+ *   divide by ub_replica_stats::n_completed for the attainment.  threshold_us, met: host [n_replicas][n].
+ * Both synchronise. */
+int  ub_percentile_curve(ub_sim*, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out_us);
+int  ub_slo_attainment(ub_sim*, uint32_t which, const int64_t* threshold_us, uint32_t n, uint32_t* met);
+
 /* gamma-Ada (Eq. 9, UPDATEGAMMA PAPER.md:588-601; rule M13 of DESIGN.md),
  * integer-only so that schedules stay bit-exact.  gamma is kept as gamma_u = gamma * 1e6.  At the start of an executed
  * iteration of an adaptive replica, if a request completed since the last update and >= min_samples have completed:

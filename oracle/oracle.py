@@ -85,6 +85,8 @@ def lib():
         L.orc_percentile_nearest_rank.argtypes = [C.c_void_p, I64, I64]; L.orc_percentile_nearest_rank.restype = I64
         L.orc_tbt_bin.argtypes = [I64]; L.orc_tbt_bin.restype = I64
         L.orc_tbt_edge.argtypes = [I64]; L.orc_tbt_edge.restype = I64
+        L.orc_percentile_curve.argtypes = [C.c_void_p, I64, C.c_void_p, I64, C.c_void_p]
+        L.orc_slo_attainment.argtypes = [C.c_void_p, I64, C.c_void_p, I64, C.c_void_p]
         L.orc_set_gamma_ada.argtypes = [C.c_void_p, P(OrcGammaAda), C.c_void_p]
         L.orc_gamma_state.argtypes = [C.c_void_p, I64, P(I64), P(I64), P(I64)]
         L.orc_gamma_grid.argtypes = [C.c_void_p, C.c_void_p]
@@ -165,6 +167,19 @@ class OracleSim:
             reps[r].gamma = float(replicas["gamma"][r])
         _chk(L.orc_set_replicas(h, reps))
         self.R, self.N, self.Q = R, int(sim["max_requests"]), int(sim["queue_cap"])
+
+    def percentile_curve(self, which, permille):
+        pm = np.ascontiguousarray(permille, np.int64)
+        out = np.zeros((self.R, len(pm)), np.int64)
+        _chk(lib().orc_percentile_curve(self._h, int(which), pm.ctypes.data, len(pm), out.ctypes.data))
+        return out
+
+    def slo_attainment(self, which, threshold_us):
+        thr = np.ascontiguousarray(threshold_us, np.int64)
+        assert thr.ndim == 2 and thr.shape[0] == self.R
+        out = np.zeros(thr.shape, np.int64)
+        _chk(lib().orc_slo_attainment(self._h, int(which), thr.ctypes.data, thr.shape[1], out.ctypes.data))
+        return out
 
     def set_gamma_ada(self, ada: dict, adaptive):
         """gamma-Ada (M13): ada = dict(window, min_samples, beta_shift, levels, gamma_min, gamma_max, eps_us)."""

@@ -676,6 +676,54 @@ int orc_per_request(orc_sim* s, int64_t* tf, int64_t* tl, uint32_t* ne, uint32_t
   return ORC_OK;
 }
 
+/* ---------- richer reductions (next row 3) ---------- */
+
+/* latencies (which: 0 TTFT = t_first - a, 1 TTLT = t_last - a) of the completed requests of one replica */
+static int64_t collect_latencies(const orc_sim* s, const orc_rep* x, int64_t which, int64_t* out) {
+  const int64_t N = s->cfg.max_requests, tr = x->par.trace_id, nreq = s->n_req[tr];
+  int64_t m = 0;
+  for (int64_t i = 0; i < nreq; i++)
+    if (x->req[i].completed)
+      out[m++] = (which == 0 ? x->req[i].t_first : x->req[i].t_last) - s->arrival[tr * N + i];
+  return m;
+}
+
+int orc_percentile_curve(orc_sim* s, int64_t which, const int64_t* permille, int64_t n, int64_t* out) {
+  if (!s || !s->have_reps || !permille || !out || which < 0 || which > 1 || n < 1) return ORC_EINVAL;
+  int64_t* v = (int64_t*)malloc(sizeof(int64_t) * (size_t)(s->cfg.max_requests > 0 ? s->cfg.max_requests : 1));
+  if (!v) return ORC_ENOMEM;
+  for (int64_t r = 0; r < s->cfg.n_replicas; r++) {
+    int64_t m = collect_latencies(s, &s->rep[r], which, v);
+    qsort(v, (size_t)m, sizeof(int64_t), i64_cmp_);
+    for (int64_t k = 0; k < n; k++) {
+      if (permille[k] < 1 || permille[k] > 1000) { free(v); return ORC_EINVAL; }
+      if (m == 0) { out[r * n + k] = 0; continue; }
+      int64_t rank = (permille[k] * m + 999) / 1000;      /* ceil(p m / 1000), 1-based */
+      if (rank < 1) rank = 1;
+      if (rank > m) rank = m;
+      out[r * n + k] = v[rank - 1];
+    }
+  }
+  free(v);
+  return ORC_OK;
+}
+
+int orc_slo_attainment(orc_sim* s, int64_t which, const int64_t* thr, int64_t n, int64_t* met) {
+  if (!s || !s->have_reps || !thr || !met || which < 0 || which > 1 || n < 1) return ORC_EINVAL;
+  int64_t* v = (int64_t*)malloc(sizeof(int64_t) * (size_t)(s->cfg.max_requests > 0 ? s->cfg.max_requests : 1));
+  if (!v) return ORC_ENOMEM;
+  for (int64_t r = 0; r < s->cfg.n_replicas; r++) {
+    int64_t m = collect_latencies(s, &s->rep[r], which, v);
+    for (int64_t k = 0; k < n; k++) {
+      int64_t c = 0;
+      for (int64_t i = 0; i < m; i++) if (v[i] <= thr[r * n + k]) c++;
+      met[r * n + k] = c;
+    }
+  }
+  free(v);
+  return ORC_OK;
+}
+
 int orc_digest(orc_sim* s, uint64_t* dg) {
   if (!s || !dg) return ORC_EINVAL;
   if (!s->have_reps) return ORC_ESTATE;

@@ -137,6 +137,11 @@ int  orc_stats_get(orc_sim*, orc_stats* out /* [R] */);
 int  orc_per_request(orc_sim*, int64_t* t_first_us, int64_t* t_last_us,
                      uint32_t* n_evict, uint32_t* n_evict_unforced /* each [R][N], nullable */);
 int  orc_digest(orc_sim*, uint64_t* digest /* [R] */);
+/* Richer reductions over the completed requests of each replica; which: 0 TTFT, 1 TTLT.
+ * Percentile curve (Fig. 6): the ceil(p m / 1000)-th smallest of the m samples (t_p of PAPER.md:225).
+ * SLO attainment (Fig. 8): number of samples <= threshold, per replica and threshold. */
+int  orc_percentile_curve(orc_sim*, int64_t which, const int64_t* permille /* [n] */, int64_t n, int64_t* out_us /* [R][n] */);
+int  orc_slo_attainment(orc_sim*, int64_t which, const int64_t* threshold_us /* [R][n] */, int64_t n, int64_t* met /* [R][n] */);
 int  orc_boost_lut(orc_sim*, int64_t replica, int64_t* lut /* [cap] */, int64_t cap, int64_t* nb);
 int  orc_tbt_hist(orc_sim*, int64_t replica, uint32_t* hist /* [4352] */);
 /* stand-alone helpers exposed so the pins can hit them directly */

@@ -57,6 +57,7 @@ class UbGammaAda(C.Structure):
 EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_step", "ub_run", "ub_stats",
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
            "ub_last_step_timing", "ub_set_iters_per_launch", "ub_set_gamma_ada", "ub_gamma_state", "ub_gamma_grid",
+           "ub_percentile_curve", "ub_slo_attainment",
            "ub_strerror")
 
 _lib = None
@@ -86,6 +87,8 @@ def lib():
         L.ub_debug_get_state.argtypes = [vp, U32, P(U32), vp, vp, vp, vp, P(I64)]
         L.ub_last_step_timing.argtypes = [vp, P(C.c_float), P(U32)]
         L.ub_set_iters_per_launch.argtypes = [vp, U32]
+        L.ub_percentile_curve.argtypes = [vp, U32, vp, U32, vp]
+        L.ub_slo_attainment.argtypes = [vp, U32, vp, U32, vp]
         L.ub_set_gamma_ada.argtypes = [vp, P(UbGammaAda), vp]
         L.ub_gamma_state.argtypes = [vp, U32, P(I64), P(C.c_int32), P(U64)]
         L.ub_gamma_grid.argtypes = [vp, vp]
@@ -247,6 +250,21 @@ class Sim:
 
     def run(self, max_iters=1 << 40, check=True):
         return ub_run(self._h, max_iters, check)
+
+    def percentile_curve(self, which, permille):
+        """[R][n] int64 microseconds: nearest-rank percentiles of TTFT (which=0) / TTLT (1) at per-mille points."""
+        pm = np.ascontiguousarray(permille, np.uint32)
+        out = np.zeros((self.R, len(pm)), np.int64)
+        _chk(lib().ub_percentile_curve(self._h, int(which), pm.ctypes.data, len(pm), out.ctypes.data))
+        return out
+
+    def slo_attainment(self, which, threshold_us):
+        """[R][n] uint32: completed requests with latency <= threshold_us[r][k]."""
+        thr = np.ascontiguousarray(threshold_us, np.int64)
+        assert thr.ndim == 2 and thr.shape[0] == self.R
+        out = np.zeros(thr.shape, np.uint32)
+        _chk(lib().ub_slo_attainment(self._h, int(which), thr.ctypes.data, thr.shape[1], out.ctypes.data))
+        return out
 
     def set_gamma_ada(self, ada: dict, adaptive):
         assert len(adaptive) == self.R

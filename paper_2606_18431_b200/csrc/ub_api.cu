@@ -539,6 +539,43 @@ int ub_stats(ub_sim* s, ub_replica_stats* out) {
   return UB_OK;
 }
 
+int ub_percentile_curve(ub_sim* s, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out) {
+  if (!s || !permille || !out || which > 1 || n < 1 || n > 16) return UB_EINVAL;
+  for (uint32_t k = 0; k < n; k++) if (permille[k] < 1 || permille[k] > 1000) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t R = s->cfg.n_replicas;
+  int64_t* d_out = nullptr;
+  int rc = dmalloc(&d_out, R * n); if (rc) return rc;
+  launch_percentile_curve(s->dev, which, permille, n, d_out, s->stream);
+  cudaError_t e = cudaMemcpyAsync(out, d_out, R * n * 8, cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(d_out);
+  if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  return UB_OK;
+}
+
+int ub_slo_attainment(ub_sim* s, uint32_t which, const int64_t* thr, uint32_t n, uint32_t* met) {
+  if (!s || !thr || !met || which > 1 || n < 1 || n > 16) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t R = s->cfg.n_replicas;
+  int64_t* d_thr = nullptr; uint32_t* d_met = nullptr;
+  int rc = UB_OK;
+  if ((rc = dmalloc(&d_thr, R * n)) || (rc = dmalloc(&d_met, R * n))) { cudaFree(d_thr); cudaFree(d_met); return rc; }
+  cudaError_t e = cudaMemcpyAsync(d_thr, thr, R * n * 8, cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) {
+    launch_slo_count(s->dev, which, n, d_thr, d_met, s->stream);
+    e = cudaMemcpyAsync(met, d_met, R * n * 4, cudaMemcpyDeviceToHost, s->stream);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(d_thr); cudaFree(d_met);
+  if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  return UB_OK;
+}
+
 __global__ void k_mask_done(const uint32_t* in, uint32_t* out, size_t n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     out[i] = in[i] & 0x7FFFFFFFu;

@@ -153,11 +153,51 @@ __device__ __forceinline__ int64_t tbt_edge(uint32_t idx) {
   return (int64_t)(idx - 128u * (uint32_t)sft) << sft;
 }
 
+struct SelectSmem { uint32_t hist[256]; uint32_t wtot[kStatThreads / 32]; unsigned long long prefix; uint32_t rank; };
+
+// The rank0-th smallest (0-based) of { src[i] - TR[i].a : request i completed }: MSD radix select, whole CTA.
+__device__ int64_t radix_select(SelectSmem& sm, const int64_t* src, const Rec0* TR, const uint32_t* ne, uint32_t nreq,
+                                uint32_t rank0) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) { sm.prefix = 0ull; sm.rank = rank0; }
+  for (int pass = 7; pass >= 0; pass--) {
+    sm.hist[tid] = 0;
+    __syncthreads();
+    const unsigned long long prefix = sm.prefix;
+    const int sh_hi = 8 * (pass + 1);
+    for (uint32_t i = tid; i < nreq; i += kStatThreads) {
+      if (!(ne[i] & kDoneBit)) continue;
+      const unsigned long long v = (unsigned long long)(src[i] - TR[i].a);
+      const bool match = (pass == 7) || ((v >> sh_hi) == (prefix >> sh_hi));
+      if (match) atomicAdd(&sm.hist[(v >> (8 * pass)) & 0xFF], 1u);
+    }
+    __syncthreads();
+    // bucket holding the rank-th (0-based) matching value: thread b owns bucket b
+    const uint32_t cntb = sm.hist[tid];
+    uint32_t inc = cntb;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += x; }
+    if (lane == 31) sm.wtot[warp] = inc;
+    __syncthreads();
+    uint32_t off = 0;
+    for (int w = 0; w < warp; w++) off += sm.wtot[w];
+    inc += off;
+    const uint32_t exc = inc - cntb, want = sm.rank;
+    __syncthreads();
+    if (want >= exc && want < inc) {
+      sm.prefix = prefix | ((unsigned long long)tid << (8 * pass));
+      sm.rank = want - exc;
+    }
+    __syncthreads();
+  }
+  const int64_t result = (int64_t)sm.prefix;
+  __syncthreads();
+  return result;
+}
+
 __global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out) {
-  __shared__ uint32_t hist[256];
+  __shared__ SelectSmem sm;
   __shared__ uint32_t wtot[kStatThreads / 32];
-  __shared__ unsigned long long sel_prefix;
-  __shared__ uint32_t sel_rank;
   const uint32_t r = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t tr = s.par[r].trace_id, nreq = s.n_req[tr];
@@ -176,41 +216,9 @@ __global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out)
         uint64_t rank = ((uint64_t)pct[k] * m + 99) / 100;
         if (rank < 1) rank = 1;
         if (rank > m) rank = m;
-        if (tid == 0) { sel_prefix = 0ull; sel_rank = (uint32_t)(rank - 1); }
-        for (int pass = 7; pass >= 0; pass--) {
-          hist[tid] = 0;
-          __syncthreads();
-          const unsigned long long prefix = sel_prefix;
-          const int sh_hi = 8 * (pass + 1);
-          for (uint32_t i = tid; i < nreq; i += kStatThreads) {
-            if (!(ne[i] & kDoneBit)) continue;
-            const unsigned long long v = (unsigned long long)(src[i] - TR[i].a);
-            const bool match = (pass == 7) || ((v >> sh_hi) == (prefix >> sh_hi));
-            if (match) atomicAdd(&hist[(v >> (8 * pass)) & 0xFF], 1u);
-          }
-          __syncthreads();
-          // bucket holding the sel_rank-th (0-based) matching value: thread b owns bucket b
-          const uint32_t cntb = hist[tid];
-          uint32_t inc = cntb;
-#pragma unroll
-          for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += x; }
-          if (lane == 31) wtot[warp] = inc;
-          __syncthreads();
-          uint32_t off = 0;
-          for (int w = 0; w < warp; w++) off += wtot[w];
-          inc += off;
-          const uint32_t exc = inc - cntb, want = sel_rank;
-          __syncthreads();
-          if (want >= exc && want < inc) {
-            sel_prefix = prefix | ((unsigned long long)tid << (8 * pass));
-            sel_rank = want - exc;
-          }
-          __syncthreads();
-        }
-        result = (int64_t)sel_prefix;
+        result = radix_select(sm, src, TR, ne, nreq, (uint32_t)(rank - 1));
       }
       if (tid == 0) { if (which == 0) out[r].ttft[k] = result; else out[r].ttlt[k] = result; }
-      __syncthreads();
     }
   }
 
@@ -247,6 +255,70 @@ __global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out)
 }
 
 void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st) { k_stats<<<s.R, kStatThreads, 0, st>>>(s, out); }
+
+// ------------------------------------------------------------------ richer reductions
+// Percentile curves (Fig. 6): nearest-rank percentiles at arbitrary per-mille points, rank =
+// ceil(p m / 1000) (t_p of PAPER.md:225), of TTFT (which = 0) or TTLT (which = 1) over a replica's completed requests.
+struct CurveArgs { uint32_t which, n; uint32_t permille[16]; };
+__global__ void __launch_bounds__(kStatThreads) k_percentile_curve(SimDev s, CurveArgs c, int64_t* out) {
+  __shared__ SelectSmem sm;
+  const uint32_t r = blockIdx.x;
+  const uint32_t tr = s.par[r].trace_id, nreq = s.n_req[tr];
+  const Rec0* TR = s.TR + (size_t)tr * s.N;
+  const int64_t* src = (c.which == 0 ? s.t_first : s.t_last) + (size_t)r * s.N;
+  const uint32_t* ne = s.n_evict + (size_t)r * s.N;
+  const uint32_t m = s.hdr[r].n_completed;
+  for (uint32_t k = 0; k < c.n; k++) {
+    int64_t result = 0;
+    if (m > 0) {
+      uint64_t rank = ((uint64_t)c.permille[k] * m + 999) / 1000;
+      if (rank < 1) rank = 1;
+      if (rank > m) rank = m;
+      result = radix_select(sm, src, TR, ne, nreq, (uint32_t)(rank - 1));
+    }
+    if (threadIdx.x == 0) out[(size_t)r * c.n + k] = result;
+  }
+}
+void launch_percentile_curve(const SimDev& s, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out,
+                             cudaStream_t st) {
+  CurveArgs c; c.which = which; c.n = n;
+  for (uint32_t k = 0; k < 16; k++) c.permille[k] = k < n ? permille[k] : 0;
+  k_percentile_curve<<<s.R, kStatThreads, 0, st>>>(s, c, out);
+}
+
+// SLO attainment (Fig. 8): per replica and threshold, the number of completed requests whose
+// latency is <= the threshold (the caller forms thresholds = SLO scale x base latency).  thr: [R][n] device.
+__global__ void __launch_bounds__(kStatThreads) k_slo_count(SimDev s, uint32_t which, uint32_t n, const int64_t* thr,
+                                                            uint32_t* out) {
+  __shared__ uint32_t cnt[16];
+  const uint32_t r = blockIdx.x;
+  const uint32_t tr = s.par[r].trace_id, nreq = s.n_req[tr];
+  const Rec0* TR = s.TR + (size_t)tr * s.N;
+  const int64_t* src = (which == 0 ? s.t_first : s.t_last) + (size_t)r * s.N;
+  const uint32_t* ne = s.n_evict + (size_t)r * s.N;
+  if (threadIdx.x < 16) cnt[threadIdx.x] = 0;
+  __syncthreads();
+  uint32_t loc[16];
+#pragma unroll
+  for (int k = 0; k < 16; k++) loc[k] = 0;
+  for (uint32_t i = threadIdx.x; i < nreq; i += kStatThreads) {
+    if (!(ne[i] & kDoneBit)) continue;
+    const int64_t v = src[i] - TR[i].a;
+#pragma unroll
+    for (int k = 0; k < 16; k++) if ((uint32_t)k < n && v <= thr[(size_t)r * n + k]) loc[k]++;
+  }
+#pragma unroll
+  for (int k = 0; k < 16; k++) {
+    const uint32_t t = __reduce_add_sync(0xffffffffu, loc[k]);
+    if ((threadIdx.x & 31) == 0 && t) atomicAdd(&cnt[k], t);
+  }
+  __syncthreads();
+  if (threadIdx.x < n) out[(size_t)r * n + threadIdx.x] = cnt[threadIdx.x];
+}
+void launch_slo_count(const SimDev& s, uint32_t which, uint32_t n, const int64_t* thr, uint32_t* out, cudaStream_t st) {
+  k_slo_count<<<s.R, kStatThreads, 0, st>>>(s, which, n, thr, out);
+}
+
 size_t stats_smem_bytes(uint32_t) { return 0; }
 int stats_configure(uint32_t) { return 0; }
 

@@ -106,6 +106,9 @@ struct StatsDev {               // device-side result of the percentile reductio
   int64_t ttft[3], ttlt[3], tbt[3];
 };
 void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st);
+void launch_percentile_curve(const SimDev& s, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out,
+                             cudaStream_t st);
+void launch_slo_count(const SimDev& s, uint32_t which, uint32_t n, const int64_t* thr, uint32_t* out, cudaStream_t st);
 size_t stats_smem_bytes(uint32_t N);
 int  stats_configure(uint32_t N);
 
