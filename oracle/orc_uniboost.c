@@ -213,7 +213,7 @@ int orc_set_replicas(orc_sim* s, const orc_replica* reps) {
   for (int64_t r = 0; r < R; r++) {
     const orc_replica* q = &reps[r];
     if (q->trace_id < 0 || q->trace_id >= c->n_traces) return ORC_EINVAL;
-    if (q->policy < 0 || q->policy > 3 || q->signal_mode < 0 || q->signal_mode > 2 ||
+    if (q->policy < 0 || q->policy > 5 || q->signal_mode < 0 || q->signal_mode > 2 ||
         q->quant_mode < 0 || q->quant_mode > 1 || q->hysteresis_us < 0 ||
         q->hysteresis_us > ((int64_t)1 << 60))
       return ORC_EINVAL;
@@ -415,6 +415,9 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
     if (x->par.policy == ORC_FCFS) key = A[id];
     else if (x->par.policy == ORC_SRPT) key = D - q->d;
     else if (x->par.policy == ORC_LAS) key = sig;
+    /* baselines of PAPER.md:51, 239 as static keys: shortest job (output length, perfect) / shortest prompt first */
+    else if (x->par.policy == ORC_SJF) key = D;
+    else if (x->par.policy == ORC_SPF) key = P;
     else key = A[id] - x->lut[bin < x->nb ? bin : x->nb - 1];
     /* Eq. 7 hysteresis as a bias on requests that hold the device */
     if (q->resident && (x->par.policy == ORC_FCFS || x->par.policy == ORC_BOOST)) key -= x->par.hysteresis_us;

@@ -228,7 +228,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   bool any_exact = false;
   for (size_t r = 0; r < R; r++) {
     const ub_replica& q = reps[r];
-    if (q.trace_id >= c.n_traces || q.policy > 3 || q.signal_mode > 2 || q.quant_mode > 1 || q.guard > 1 ||
+    if (q.trace_id >= c.n_traces || q.policy > 5 || q.signal_mode > 2 || q.quant_mode > 1 || q.guard > 1 ||
         q.hysteresis_us < 0 || q.hysteresis_us > (1ll << 60))
       return UB_EINVAL;
     if (q.policy == UB_BOOST && !(q.gamma > 0.0)) return UB_EINVAL;     // also rejects NaN

@@ -225,6 +225,8 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         if (par.policy == 0) kv = r0[c].a;
         else if (par.policy == 1) kv = (int64_t)(r0[c].D - r1[c].d);
         else if (par.policy == 3) kv = (int64_t)sig;
+        else if (par.policy == 4) kv = (int64_t)r0[c].D;                               // SJF, perfect lengths
+        else if (par.policy == 5) kv = (int64_t)r0[c].P;                               // SPF
         else kv = r0[c].a - __ldg(lut + (bin < par.lut_nb ? bin : par.lut_nb - 1));   // pi = a - b
         const bool res = (r1[c].flags & F_RESIDENT) != 0;
         if (res && (par.policy == 0 || par.policy == 2)) kv -= par.delta;             // Eq. 7 as a bias

@@ -101,7 +101,8 @@ def test_config1_step_by_step(gpu, oracle_mod):
 
 # ------------------------------------------------------------------------------------------ memory pressure
 
-@pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS])
+@pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS, W.POLICY_SJF,
+                                    W.POLICY_SPF])
 @pytest.mark.parametrize("preempt", [W.PRE_RECOMPUTE, W.PRE_SWAP, W.PRE_AUTO])
 def test_pressure_policies_preemption(gpu, oracle_mod, policy, preempt):
     for seed in range(4):

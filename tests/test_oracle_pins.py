@@ -436,6 +436,52 @@ def test_bruteforce_tiny_traces(seed):
     assert int(res[W.POLICY_FCFS].max()) == opt_max
 
 
+# ------------------------------------------------------------------ baselines SJF / SPF as static keys
+
+@pytest.mark.parametrize("seed", range(20))
+def test_sjf_spf_are_shortest_processing_time_first(seed):
+    """Single server, all jobs present at time 0: shortest-processing-time-first minimises the total completion time
+    (Smith's rule, 1 || sum C_j).  SJF sees job size = output length D (one token per slot); SPF sees job size =
+    prompt length P (one prefill token per slot, single-token outputs).  Both must attain the brute-force optimum
+    over ALL slot schedules, which is also the closed form sum_k (n - k) s_(k) over the sorted sizes."""
+    rng = np.random.default_rng([14, seed])
+    n = int(rng.integers(2, 6))
+    size = [int(x) for x in rng.integers(1, 5, n)]
+    c0 = 1000
+    opt_sum, _ = _brute_optima(tuple([0] * n), size)
+    closed = sum((n - k) * v for k, v in enumerate(sorted(size)))
+    assert opt_sum == closed
+    sjf = W.custom(np.zeros(n, np.int64), np.ones(n, np.int32), size, dict(
+        max_batch=1, kv_blocks=1 << 16, c0_us=c0, c_prefill_tok_us=0, c_decode_seq_us=0, queue_cap=n),
+        W.make_replicas(1, policy=W.POLICY_SJF, guard=0, hysteresis_us=0))
+    spf = W.custom(np.zeros(n, np.int64), size, np.ones(n, np.int32), dict(
+        max_batch=1, chunk_tokens=1, token_budget=1, kv_blocks=1 << 16, c0_us=c0, c_prefill_tok_us=0,
+        c_decode_seq_us=0, queue_cap=n),
+        W.make_replicas(1, policy=W.POLICY_SPF, guard=0, hysteresis_us=0))
+    for wl in (sjf, spf):
+        sim = run_wl(wl)
+        _, tl, _, _ = sim.per_request()
+        assert (tl[0, :n] % c0 == 0).all()
+        assert int(tl[0, :n].sum()) // c0 == opt_sum
+        # the completion order is the size order (ties by id)
+        assert list(np.argsort(tl[0, :n], kind="stable")) == sorted(range(n), key=lambda i: (size[i], i))
+
+
+def test_sjf_preempts_by_total_length_not_by_remaining():
+    """A static key: a job of length 3 arriving while a job of length 4 has 1 token left still preempts it (SRPT
+    would not) -- the difference between SJF with perfect lengths and SRPT."""
+    c0 = 1000
+    arr, D = np.array([0, 3]) * c0, [4, 3]
+    out = {}
+    for pol in (W.POLICY_SJF, W.POLICY_SRPT):
+        wl = W.custom(arr, np.ones(2, np.int32), D, dict(
+            max_batch=1, kv_blocks=1 << 16, c0_us=c0, c_prefill_tok_us=0, c_decode_seq_us=0, queue_cap=2),
+            W.make_replicas(1, policy=pol, guard=0, hysteresis_us=0))
+        out[pol] = [int(x) // c0 for x in run_wl(wl).per_request()[1][0, :2]]
+    assert out[W.POLICY_SJF] == [7, 6]        # job 0 runs slots 0-2, waits for job 1 (slots 3-5), finishes in slot 6
+    assert out[W.POLICY_SRPT] == [4, 7]       # job 0 (1 left) keeps the server, job 1 runs slots 4-6
+
+
 # ------------------------------------------------------------------ P10 Eq. 6 arg-min subset
 
 @pytest.mark.parametrize("seed", range(10))
@@ -470,7 +516,7 @@ def test_admitted_set_is_argmin_subset(seed):
 # ------------------------------------------------------------------ P11 MemGuard logarithmic bound
 
 @pytest.mark.parametrize("seed", range(8))
-@pytest.mark.parametrize("policy", [W.POLICY_BOOST, W.POLICY_SRPT, W.POLICY_LAS])
+@pytest.mark.parametrize("policy", [W.POLICY_BOOST, W.POLICY_SRPT, W.POLICY_LAS, W.POLICY_SJF, W.POLICY_SPF])
 def test_memguard_logarithmic_preemption_bound(seed, policy):
     """'request i can trigger at most 1 + floor(log2(S_i/k)) priority-revision points' (PAPER.md:213-215):
     evictions of a request that was not locked (unforced) are bounded by that number."""
