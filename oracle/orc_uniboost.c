@@ -213,11 +213,11 @@ int orc_set_replicas(orc_sim* s, const orc_replica* reps) {
   for (int64_t r = 0; r < R; r++) {
     const orc_replica* q = &reps[r];
     if (q->trace_id < 0 || q->trace_id >= c->n_traces) return ORC_EINVAL;
-    if (q->policy < 0 || q->policy > 5 || q->signal_mode < 0 || q->signal_mode > 2 ||
+    if (q->policy < 0 || q->policy > 6 || q->signal_mode < 0 || q->signal_mode > 2 ||
         q->quant_mode < 0 || q->quant_mode > 1 || q->hysteresis_us < 0 ||
         q->hysteresis_us > ((int64_t)1 << 60))
       return ORC_EINVAL;
-    if (q->policy == ORC_BOOST && !(q->gamma > 0.0)) return ORC_EINVAL; /* also rejects NaN */
+    if ((q->policy == ORC_BOOST || q->policy == ORC_DISTBOOST) && !(q->gamma > 0.0)) return ORC_EINVAL; /* also rejects NaN */
   }
   free_reps(s);
   s->rep = (orc_rep*)calloc((size_t)R, sizeof(orc_rep));
@@ -245,7 +245,7 @@ int orc_set_replicas(orc_sim* s, const orc_replica* reps) {
     x->lut = (int64_t*)calloc((size_t)nb, sizeof(int64_t));
     if (!x->lut) return ORC_ENOMEM;
     for (int64_t b = 0; b < nb; b++) {
-      if (x->par.policy != ORC_BOOST) { x->lut[b] = 0; continue; }
+      if (x->par.policy != ORC_BOOST && x->par.policy != ORC_DISTBOOST) { x->lut[b] = 0; continue; }
       /* w_hat = k * 2^b (Eq. 8), in fp64 so that absurd bins cannot overflow */
       double what = (x->par.quant_mode == ORC_Q_EXACT) ? (double)b : ldexp((double)c->bin_tokens, (int)b);
       x->lut[b] = boost_fixed(x->par.gamma, what, c->tok_us);
@@ -418,11 +418,22 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
     /* baselines of PAPER.md:51, 239 as static keys: shortest job (output length, perfect) / shortest prompt first */
     else if (x->par.policy == ORC_SJF) key = D;
     else if (x->par.policy == ORC_SPF) key = P;
+    else if (x->par.policy == ORC_DISTBOOST) {
+      /* DistBoost (M14): decode queue Q_d = {prefill done} keyed by the time of entering it, Eq. 4; prefill queue
+         keyed by a - b_gamma(s_pre), Eq. 3 */
+      if (q->d >= 1) key = q->t_first;
+      else {
+        int64_t pb = (x->par.quant_mode == ORC_Q_GEOMETRIC) ? orc_quant_bin(P, c->bin_tokens) : P;
+        key = A[id] - x->lut[pb < x->nb ? pb : x->nb - 1];
+      }
+    }
     else key = A[id] - x->lut[bin < x->nb ? bin : x->nb - 1];
     /* Eq. 7 hysteresis as a bias on requests that hold the device */
     if (q->resident && (x->par.policy == ORC_FCFS || x->par.policy == ORC_BOOST)) key -= x->par.hysteresis_us;
     /* MemGuard minimum-run lock: dispatched and still in the bin it was locked at */
     int64_t klass = (x->par.guard && q->resident && bin == q->lockbin) ? 0 : 1;
+    /* DistBoost: the decode batch is selected first, prefill piggybacks on what is left (Eq. 5-6) */
+    if (x->par.policy == ORC_DISTBOOST) klass = (q->d >= 1) ? 0 : 1;
     e[j].klass = klass; e[j].key = key; e[j].id = id; e[j].bin = bin;
     e[j].resident_before = q->resident; e[j].want = 0; e[j].evict = 0;
   }

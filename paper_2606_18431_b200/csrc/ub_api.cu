@@ -228,10 +228,10 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   bool any_exact = false;
   for (size_t r = 0; r < R; r++) {
     const ub_replica& q = reps[r];
-    if (q.trace_id >= c.n_traces || q.policy > 5 || q.signal_mode > 2 || q.quant_mode > 1 || q.guard > 1 ||
+    if (q.trace_id >= c.n_traces || q.policy > 6 || q.signal_mode > 2 || q.quant_mode > 1 || q.guard > 1 ||
         q.hysteresis_us < 0 || q.hysteresis_us > (1ll << 60))
       return UB_EINVAL;
-    if (q.policy == UB_BOOST && !(q.gamma > 0.0)) return UB_EINVAL;     // also rejects NaN
+    if ((q.policy == UB_BOOST || q.policy == UB_DISTBOOST) && !(q.gamma > 0.0)) return UB_EINVAL;     // also rejects NaN
     any_exact |= (q.quant_mode == UB_Q_EXACT);
   }
   s->have_reps = false;
@@ -258,7 +258,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
     const ub_replica& q = reps[r];
     const uint32_t nb = (q.quant_mode == UB_Q_EXACT) ? s->h_maxsig[q.trace_id] + 1u : 64u;
     uint32_t off = 0;
-    if (q.policy == UB_BOOST) {
+    if (q.policy == UB_BOOST || q.policy == UB_DISTBOOST) {
       uint64_t gb; memcpy(&gb, &q.gamma, 8);
       auto key = std::make_tuple(gb, (uint32_t)q.quant_mode, nb);
       auto it = seen.find(key);
@@ -621,7 +621,7 @@ int ub_boost_lut(ub_sim* s, uint32_t r, int64_t* lut, uint32_t cap, uint32_t* nb
   const uint32_t n = s->h_lut_nb[r];
   *nb = n;
   if (lut) {
-    const bool boost = s->h_reps[r].policy == UB_BOOST;
+    const bool boost = s->h_reps[r].policy == UB_BOOST || s->h_reps[r].policy == UB_DISTBOOST;
     for (uint32_t b = 0; b < n && b < cap; b++) lut[b] = boost ? s->h_lut[s->h_lut_off[r] + b] : 0;
   }
   return UB_OK;

@@ -227,11 +227,16 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         else if (par.policy == 3) kv = (int64_t)sig;
         else if (par.policy == 4) kv = (int64_t)r0[c].D;                               // SJF, perfect lengths
         else if (par.policy == 5) kv = (int64_t)r0[c].P;                               // SPF
+        else if (par.policy == 6) {                                                    // DistBoost (M14), Eq. 3-4
+          if (r1[c].d >= 1u) kv = __ldcg(g_tfirst + r1[c].id);
+          else { const uint32_t pb = bin_of(par, s.k, r0[c].P); kv = r0[c].a - __ldg(lut + (pb < par.lut_nb ? pb : par.lut_nb - 1)); }
+        }
         else kv = r0[c].a - __ldg(lut + (bin < par.lut_nb ? bin : par.lut_nb - 1));   // pi = a - b
         const bool res = (r1[c].flags & F_RESIDENT) != 0;
         if (res && (par.policy == 0 || par.policy == 2)) kv -= par.delta;             // Eq. 7 as a bias
         const uint32_t lockp1 = r1[c].flags >> F_LOCK_SHIFT;
-        const uint64_t klass = (par.guard && res && lockp1 == bin + 1u) ? 0ull : 1ull;
+        uint64_t klass = (par.guard && res && lockp1 == bin + 1u) ? 0ull : 1ull;
+        if (par.policy == 6) klass = r1[c].d >= 1u ? 0ull : 1ull;                     // decode batch first, Eq. 5-6
         key[c] = (klass << 63) | (uint64_t)(kv + kKeyBias);
         const uint32_t dirty = (r1[c].flags & F_DIRTY) ? 1u : 0u;
         n_dirty += dirty;
@@ -576,7 +581,8 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         uint32_t bin2 = bin;
         if (r1[c].d != d_old) bin2 = bin_of(par, s.k, signal_of(par, r0[c].P, r0[c].D, r1[c].d));
         const bool res2 = (nf & F_RESIDENT) != 0;
-        const uint32_t klass2 = (par.guard && res2 && bin2 == bin) ? 0u : 1u;
+        uint32_t klass2 = (par.guard && res2 && bin2 == bin) ? 0u : 1u;
+        if (par.policy == 6) klass2 = r1[c].d >= 1u ? 0u : 1u;                         // DistBoost: phase = class
         const bool bin_matters = par.policy == 2;
         const bool dirty = (((nf ^ of) & F_RESIDENT) != 0) || (bin_matters && bin2 != bin) || (klass2 != klass);
         if (res2) nf |= (bin + 1u) << F_LOCK_SHIFT;

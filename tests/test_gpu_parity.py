@@ -102,12 +102,12 @@ def test_config1_step_by_step(gpu, oracle_mod):
 # ------------------------------------------------------------------------------------------ memory pressure
 
 @pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS, W.POLICY_SJF,
-                                    W.POLICY_SPF])
+                                    W.POLICY_SPF, W.POLICY_DISTBOOST])
 @pytest.mark.parametrize("preempt", [W.PRE_RECOMPUTE, W.PRE_SWAP, W.PRE_AUTO])
 def test_pressure_policies_preemption(gpu, oracle_mod, policy, preempt):
     for seed in range(4):
         wl = pressure_workload(seed, n=120, kv_blocks=40, policy=policy, preempt=preempt,
-                               guard=1 if policy == W.POLICY_BOOST else 0, swap_pool_blocks=24)
+                               guard=1 if policy in (W.POLICY_BOOST, W.POLICY_DISTBOOST) else 0, swap_pool_blocks=24)
         g, o = _pair(gpu, oracle_mod, wl)
         g.run(); o.run()
         _assert_same(g, o, f"pressure seed {seed} policy {policy} preempt {preempt}")

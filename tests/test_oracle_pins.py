@@ -664,3 +664,62 @@ def test_workload_generators_are_seeded_and_feasible():
     wl = W.config2(n_seeds=16)
     x = wl.traces(workers=1); y = wl.traces(workers=2)
     assert all(np.array_equal(u, v) for u, v in zip(x, y))
+
+
+# ------------------------------------------------------------------ DistBoost (Phase 1 strawman, rule M14)
+
+@pytest.mark.parametrize("seed", range(5))
+@pytest.mark.parametrize("gamma", [0.05, 3.0])
+def test_distboost_single_slot_is_non_preemptive_fifo(seed, gamma):
+    """Eq. 5 selects the decode batch first.  With one slot and one-token prompts a request enters
+    the decode queue in its first slot and then holds the server until it completes; equal prompts give equal
+    prefill boosts, so the prefill queue is FIFO: the replica is the G/G/1 FIFO queue of the Lindley recursion,
+    whatever gamma -- the inter-queue head-of-line blocking the paper describes."""
+    rng = np.random.default_rng([15, seed])
+    n, c0 = 150, 5000
+    D = rng.integers(1, 12, n)
+    a = np.cumsum(rng.exponential(30000, n)).astype(np.int64)
+    wl = W.custom(a, np.ones(n, np.int32), D, dict(
+        max_batch=1, kv_blocks=1 << 20, c0_us=c0, c_prefill_tok_us=0, c_decode_seq_us=0, queue_cap=n),
+        W.make_replicas(1, policy=W.POLICY_DISTBOOST, guard=0, hysteresis_us=0, gamma=gamma))
+    sim = run_wl(wl)
+    tf, tl, _, _ = sim.per_request()
+    C_prev = 0
+    for i in range(n):
+        start = max(int(a[i]), C_prev)
+        C_prev = start + int(D[i]) * c0
+        assert tl[0, i] == C_prev and tf[0, i] == start + c0
+
+
+def test_distboost_two_queues_eq3_to_eq6():
+    """Every iteration: the order is the decode queue (requests that emitted their first token) by the time they
+    entered it (Eq. 4), then the prefill queue by a - b_gamma(prompt) (Eq. 3); the batch is a prefix of it (Eq. 5-6)."""
+    wl = pressure_workload(3, n=120, kv_blocks=4096, policy=W.POLICY_DISTBOOST, guard=0, gamma=0.3)
+    tr = wl.traces()
+    a, P = tr[0][0], tr[1][0]
+    o = O.OracleSim(wl.sim, wl.replicas, tr)
+    first = {}
+    k, tok = int(wl.sim["bin_tokens"]), int(wl.sim["tok_us"])
+    seen_mixed = False
+    for it in range(20000):
+        info, rows = o.step_replica(0)
+        if not info["executed"]:
+            break
+        dec = [r for r in rows if r["id"] in first]
+        pre = [r for r in rows if r["id"] not in first]
+        assert [r["id"] for r in rows] == [r["id"] for r in dec] + [r["id"] for r in pre]      # decode queue first
+        assert all(r["klass"] == 0 and r["key"] == first[r["id"]] for r in dec)               # Eq. 4
+        for r in pre:                                                                          # Eq. 3
+            assert r["klass"] == 1 and r["key"] == int(a[r["id"]]) - O.boost_us(0.3, k * 2 ** O.quant_bin(int(P[r["id"]]), k), tok)
+        assert [(r["key"], r["id"]) for r in dec] == sorted((r["key"], r["id"]) for r in dec)
+        assert [(r["key"], r["id"]) for r in pre] == sorted((r["key"], r["id"]) for r in pre)
+        adm = [r["want"] > 0 for r in rows]
+        assert adm == sorted(adm, reverse=True)                                                # KV ample: a prefix
+        seen_mixed |= bool(dec) and bool(pre)
+        for r in rows:                                                                         # entering the decode queue
+            if r["id"] not in first and r["d_after"] >= 1:
+                first[r["id"]] = info["t_end_us"]
+    assert seen_mixed
+    tf = o.per_request()[0][0]
+    assert all(tf[i] == t for i, t in first.items())
+    o.close()
