@@ -266,13 +266,13 @@ def test_configs_sampled_full_run(gpu, oracle_mod, cfg_id, kw, picks):
 
 # ------------------------------------------------------------------------------------------ full sizes, sampled replicas
 
-def _full_size_sampled(gpu, oracle_mod, wl, picks):
+def _full_size_sampled(gpu, oracle_mod, wl, picks, ipl=1):
     """Run the whole workload on the GPU in bench.py's launch configuration (one iteration per launch), then compare
     the schedule digest, the counters and the integer / fp64 percentiles of the sampled replicas with the oracle,
     which computes those replicas one by one (a replica's schedule does not depend on the batch around it, P14)."""
     import os
     tr = wl.traces(workers=max(1, min(32, os.cpu_count() or 1)))
-    g = gpu.Sim(wl.sim, wl.replicas, tr, iters_per_launch=1)
+    g = gpu.Sim(wl.sim, wl.replicas, tr, iters_per_launch=ipl)
     g.run()
     dg = g.digest()
     raw = g.stats_raw()
@@ -307,3 +307,11 @@ def test_config5_full_size_sampled(gpu, oracle_mod):
     """BASELINE.json configs[4] at its full size (65536 replicas x 8192 requests; rounds split over two streams)."""
     _full_size_sampled(gpu, oracle_mod, W.config5(n_seeds=65536, n_requests=8192),
                        [0, 1, 4095, 8191, 16384, 32767, 32768, 32769, 40000, 50001, 65534, 65535])
+
+
+@pytest.mark.parametrize("ipl", [1, 16])
+def test_split_rounds_and_resident_mode(gpu, oracle_mod, ipl):
+    """8192 replicas (rounds split over two streams, ticket-based replica distribution) with 1 and with 16 iterations
+    per launch (the bench's resident-state mode): sampled replicas, both halves and their borders, against the oracle."""
+    _full_size_sampled(gpu, oracle_mod, W.config5(n_seeds=8192, n_requests=640),
+                       [0, 1, 2047, 4094, 4095, 4096, 4097, 6000, 8190, 8191], ipl=ipl)
