@@ -106,35 +106,31 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   // Work distribution: windows differ by two orders of magnitude.  A warp takes its first `nstat` replicas by static
   // striding (3/4 of an even share); the rest are handed out dynamically: each is the next value of a global ticket
   // counter (count[4], zeroed per round), requested one replica ahead so that the atomic's latency is never waited for.
-  const uint32_t gw = A.rbeg + blockIdx.x * kSWarps + wib;
-  const uint32_t share = ((A.rend - A.rbeg) / nwarps) * 3u / 4u;
-  const uint32_t nstat = share > 2u ? share : 2u;
-  const uint32_t dynbase = A.rbeg + nstat * nwarps;
-  uint32_t r = gw, rn = gw + nwarps;
+#define UB_GW (A.rbeg + blockIdx.x * kSWarps + (threadIdx.x >> 5))
+  uint32_t r = UB_GW, rn = UB_GW + nwarps;
   uint32_t taken = 2, ticket = 0;
   uint32_t parity = 0;
   prefetch_replica(r, 0);
-  for (; r < A.rend; r = rn, rn = (taken < nstat ? gw + taken * nwarps : __shfl_sync(kFull, ticket, 0) + dynbase), taken++,
+  for (; r < A.rend; r = rn, rn = (taken < A.nstat ? UB_GW + taken * nwarps : __shfl_sync(kFull, ticket, 0) + A.dynbase), taken++,
                   parity ^= 1u) {
     cp_wait<0>();
     __syncwarp();
     prefetch_replica(rn, parity ^ 1u);
-    if (taken >= nstat && lane == 0) ticket = atomicAdd(A.count + 4, 1u);
+    if (taken >= A.nstat && lane == 0) ticket = atomicAdd(A.count + 4, 1u);
     const unsigned long long* sh = reinterpret_cast<const unsigned long long*>(X.hdr[parity]);
-    unsigned long long* h64 = reinterpret_cast<unsigned long long*>(s.hdr + r);
-    const unsigned long long w13 = sh[13];
-    int64_t a_next = (int64_t)sh[2];
-    uint32_t n = (uint32_t)w13, next = (uint32_t)(w13 >> 32);
-    if (n == 0 && a_next == kNever) continue;                         // finished its trace
-    int64_t t = (int64_t)sh[0];
+    // (addresses and per-replica scalars that are needed rarely are re-derived where they are used instead of
+    // living in registers across the chunk loop)
+#define UB_H64 (reinterpret_cast<unsigned long long*>(s.hdr + r))
+#define UB_TR (s.TR + (size_t)reinterpret_cast<const RepPar*>(X.par[parity])->trace_id * s.N)
+#define UB_DELTA (reinterpret_cast<const RepPar*>(X.par[parity])->delta)
+    uint32_t n = (uint32_t)sh[13];
+    if (n == 0 && (int64_t)sh[2] == kNever) continue;                 // finished its trace
     uint32_t nd = (uint32_t)sh[18];                                   // entries of the dirty list
     const uint32_t iters = A.iters;
     const RepPar par = *reinterpret_cast<const RepPar*>(X.par[parity]);
-    const Rec0* TR = s.TR + (size_t)par.trace_id * s.N;
     Rec0* gE0 = s.E0 + (size_t)r * Q;
     Rec1* gE1 = s.E1 + (size_t)r * Q;
     const bool isboost = par.policy == 2;
-    const int64_t delta = par.delta;
     const bool guard = par.guard != 0;
 
     // the streaming path covers the arrival-keyed policies with the paper's signal and quantiser
@@ -148,15 +144,23 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 
     for (; !slow && it < iters; it++) {
       // ---------------- a0: idle jump + ingest (M6)
+      // (the clock, the next arrival and the trace cursor live in the shared-memory header image -- words 0, 2, 13 --
+      // between their few uses)
+      int64_t t = (int64_t)sh[0];
+      int64_t a_next = (int64_t)sh[2];
+      uint32_t next = (uint32_t)(sh[13] >> 32);
       if (n == 0) {
         if (a_next == kNever) break;
-        if (a_next > t) t = a_next;
+        if (a_next > t) {
+          t = a_next;
+          if (lane == 0) reinterpret_cast<unsigned long long*>(X.hdr[parity])[0] = (unsigned long long)t;
+        }
       }
       uint32_t cnt = 0, nreq = 0;
       if (a_next <= t && n < Q) {                                     // a_next != kNever => next < nreq
         nreq = __ldg(s.n_req + par.trace_id);
         const uint32_t avail = (Q - n) < (nreq - next) ? (Q - n) : (nreq - next);
-        const bool take = (uint32_t)lane < avail && __ldg(&TR[next + lane].a) <= t;   // arrivals sorted => a prefix
+        const bool take = (uint32_t)lane < avail && __ldg(&UB_TR[next + lane].a) <= t;   // arrivals sorted => a prefix
         cnt = __popc(__ballot_sync(kFull, take));
         if (cnt == 32u && avail > 32u) cnt = 64u;                     // maybe more: not for this kernel
       }
@@ -199,17 +203,23 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + spos));
         } else if ((uint32_t)lane < m) {
           const uint32_t i = next + ((uint32_t)lane - nd);
-          v0 = __ldg(reinterpret_cast<const int4*>(TR + i));
+          v0 = __ldg(reinterpret_cast<const int4*>(UB_TR + i));
           v1 = make_int4((int)i, 0, 0, 0);
         }
         if (cnt) {
           next += cnt;
-          a_next = (next < nreq) ? __ldg(&TR[next].a) : kNever;
+          a_next = (next < nreq) ? __ldg(&UB_TR[next].a) : kNever;
+          if (lane == 0) {
+            unsigned long long* shw = reinterpret_cast<unsigned long long*>(X.hdr[parity]);
+            shw[2] = (unsigned long long)a_next;
+            shw[13] = (shw[13] & 0xFFFFFFFFull) | ((unsigned long long)next << 32);
+            __stcg(UB_H64 + 2, (unsigned long long)a_next);
+          }
         }
         const Rec0 q0 = *reinterpret_cast<const Rec0*>(&v0);
         const Rec1 q1 = *reinterpret_cast<const Rec1*>(&v1);
         uint64_t sk; uint32_t sb;
-        score(q0, q1, k, lutv, delta, guard, sk, sb);
+        score(q0, q1, k, lutv, UB_DELTA, guard, sk, sb);
         uint32_t rank = 0;
         if (m > 1u) {
           for (uint32_t j = 0; j < m; j++) {
@@ -351,7 +361,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const bool defer = emitted && (d_old == 0u || !ep_old || gone);
         const bool ends = valid && !emitted && ep_old;
         if (__any_sync(kFull, defer || ends)) {
-          if (ends) s.t_last[(size_t)r * s.N + w1.id] = t;            // persist t_last when the streak ends
+          if (ends) s.t_last[(size_t)r * s.N + w1.id] = (int64_t)sh[0];   // persist t_last when the streak ends
           const uint32_t em = __ballot_sync(kFull, defer);
           if (defer)
             s.evbuf[(size_t)r * s.evcap + nev + __popc(em & ltmask)] =
@@ -403,7 +413,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           if (__all_sync(kFull, steady || !((cv >> lane) & 1u))) {
             bool before = true;
             if (pend) {
-              score(r0, r1, k, lutv, delta, guard, key, bin);
+              score(r0, r1, k, lutv, UB_DELTA, guard, key, bin);
               scored = true;
               const int last = 31 - __clz((int)cv);
               const uint64_t lk = __shfl_sync(kFull, key, last);
@@ -449,7 +459,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
             }
           }
         }
-        if (!scored) score(r0, r1, k, lutv, delta, guard, key, bin);
+        if (!scored) score(r0, r1, k, lutv, UB_DELTA, guard, key, bin);
         uint32_t lo = 0;
         for (;;) {
           uint32_t fl = 32;
@@ -562,7 +572,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       }
       const int64_t cost = s.c0 + s.c_pf * (int64_t)pf + s.c_dec * (int64_t)dec +
                            (int64_t)(((uint64_t)(swin_blocks + swout_blocks) * s.swap_ns + 500u) / 1000u);
-      const int64_t t_end = t + cost;
+      const int64_t t_end = (int64_t)sh[0] + cost;
 
       // ---------------- the queued per-request events, now that t_end is known (M10, M11)
       if (nev) {
@@ -592,14 +602,14 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
             if (ev.y & 4u) {
               g_tlast[id] = t_end;
               const int64_t tf = (ev.y & 1u) ? t_end : __ldcg(g_tfirst + id);
-              const int4 tv = __ldg(reinterpret_cast<const int4*>(TR + id));
+              const int4 tv = __ldg(reinterpret_cast<const int4*>(UB_TR + id));
               const Rec0 q0 = *reinterpret_cast<const Rec0*>(&tv);
               if constexpr (ADA)                                      // gamma-Ada: end-to-end latency sample (M13)
                 s.ada_ring[(size_t)r * s.ada_W + (cseq + __popc(cm & ltmask)) % s.ada_W] = t_end - q0.a;
-              atomicAdd(h64 + 8, (unsigned long long)(tf - q0.a));
-              atomicAdd(h64 + 9, (unsigned long long)(t_end - q0.a));
-              atomicAdd(h64 + 10, (unsigned long long)(t_end - tf));
-              atomicAdd(h64 + 11, (unsigned long long)(q0.D - 1u));
+              atomicAdd(UB_H64 + 8, (unsigned long long)(tf - q0.a));
+              atomicAdd(UB_H64 + 9, (unsigned long long)(t_end - q0.a));
+              atomicAdd(UB_H64 + 10, (unsigned long long)(t_end - tf));
+              atomicAdd(UB_H64 + 11, (unsigned long long)(q0.D - 1u));
               ev_add(evl, evu, EV_COMPLETE, id, 0u);
               uint32_t* g_ne = s.n_evict + (size_t)r * s.N;
               g_ne[id] = __ldcg(g_ne + id) | 0x80000000u;             // completion marker read by the stats kernel
@@ -617,28 +627,29 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         unsigned long long* shw = reinterpret_cast<unsigned long long*>(X.hdr[parity]);
         const uint64_t H = digest_fold(shw[1], evl, evu, t_end);
         shw[1] = H;                                                   // (kept current for a further iteration)
+        shw[0] = (unsigned long long)t_end;
         if constexpr (ADA) shw[15] += (unsigned long long)n_done | ((unsigned long long)ev_nrc << 32);
         const uint32_t pk = n > peak ? n : peak;
         shw[14] = (unsigned long long)swap_used | ((unsigned long long)pk << 32);
         if (same) atomicAdd(s.hist + (size_t)r * kTbtBins + tbt_bin(cost), same);
-        __stcg(h64 + 0, (unsigned long long)t_end);
-        __stcg(h64 + 1, (unsigned long long)H);
-        if (cnt) __stcg(h64 + 2, (unsigned long long)a_next);
-        __stcg(h64 + 13, (unsigned long long)n_new | ((unsigned long long)next << 32));
+        __stcg(UB_H64 + 0, (unsigned long long)t_end);
+        __stcg(UB_H64 + 1, (unsigned long long)H);
+        shw[13] = (unsigned long long)n_new | (shw[13] & 0xFFFFFFFF00000000ull);
+        __stcg(UB_H64 + 13, shw[13]);
         if (n > peak || swin_blocks || swout_blocks)
-          __stcg(h64 + 14, (unsigned long long)swap_used | ((unsigned long long)pk << 32));
-        if (ndnew != nd) __stcg(reinterpret_cast<uint32_t*>(h64 + 18), ndnew);
-        atomicAdd(h64 + 3, (unsigned long long)n);                    // request-steps
-        atomicAdd(h64 + 4, (unsigned long long)emit);
-        if (pf) atomicAdd(h64 + 5, (unsigned long long)pf);
-        atomicAdd(h64 + 6, (unsigned long long)dec);
-        if (ev_lost) atomicAdd(h64 + 7, (unsigned long long)ev_lost);
-        atomicAdd(h64 + 12, 1ull);                                    // iterations
-        if (n_done | ev_nrc) atomicAdd(h64 + 15, (unsigned long long)n_done | ((unsigned long long)ev_nrc << 32));
-        if (ev_nsw | swin_cnt) atomicAdd(h64 + 16, (unsigned long long)ev_nsw | ((unsigned long long)swin_cnt << 32));
+          __stcg(UB_H64 + 14, (unsigned long long)swap_used | ((unsigned long long)pk << 32));
+        if (ndnew != nd) __stcg(reinterpret_cast<uint32_t*>(UB_H64 + 18), ndnew);
+        atomicAdd(UB_H64 + 3, (unsigned long long)n);                    // request-steps
+        atomicAdd(UB_H64 + 4, (unsigned long long)emit);
+        if (pf) atomicAdd(UB_H64 + 5, (unsigned long long)pf);
+        atomicAdd(UB_H64 + 6, (unsigned long long)dec);
+        if (ev_lost) atomicAdd(UB_H64 + 7, (unsigned long long)ev_lost);
+        atomicAdd(UB_H64 + 12, 1ull);                                    // iterations
+        if (n_done | ev_nrc) atomicAdd(UB_H64 + 15, (unsigned long long)n_done | ((unsigned long long)ev_nrc << 32));
+        if (ev_nsw | swin_cnt) atomicAdd(UB_H64 + 16, (unsigned long long)ev_nsw | ((unsigned long long)swin_cnt << 32));
       }
-      t = t_end; n = n_new; wsize = n_new; nd = ndnew;
-      if (n == 0 && a_next == kNever) {                               // finished its trace in this call
+      n = n_new; wsize = n_new; nd = ndnew;
+      if (n == 0 && (int64_t)sh[2] == kNever) {                       // finished its trace in this call
         if (lane == 0) atomicAdd(A.count + 5, 1u);
         it++;
         break;
@@ -648,15 +659,20 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 
     // ---------------- not handled here: queue the replica for the team kernels of this round
     if (slow && lane == 0) {
-      if (it > 0) reinterpret_cast<uint32_t*>(h64 + 17)[1] = iters - it;       // iterations still to do
+      if (it > 0) reinterpret_cast<uint32_t*>(UB_H64 + 17)[1] = iters - it;       // iterations still to do
       push_list(A, s.all_stream ? 2u : (wsize <= A.thrS ? 0u : (wsize <= A.thrM ? 1u : 2u)), r);
     }
   }
   cp_wait<0>();
+#undef UB_H64
+#undef UB_GW
+#undef UB_TR
+#undef UB_DELTA
 }
 
 // persistent grid: every warp takes replicas until none is left
-template <bool ADA> static void launch_stream_t(const StepArgs& A, cudaStream_t st) {
+template <bool ADA> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
+  StepArgs A = A0;
   static int ctas_per_sm = 0;
   if (!ctas_per_sm) {
     cudaFuncSetAttribute(k_stream<ADA>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -670,6 +686,10 @@ template <bool ADA> static void launch_stream_t(const StepArgs& A, cudaStream_t 
   const uint32_t need = (A.rend - A.rbeg + kSWarps - 1) / kSWarps;
   uint32_t grid = (uint32_t)(sms * ctas_per_sm);
   if (grid > need) grid = need;
+  // a warp takes 3/4 of an even share of the replicas by static striding, the rest by tickets
+  const uint32_t nwarps = grid * kSWarps, share = ((A.rend - A.rbeg) / nwarps) * 3u / 4u;
+  A.nstat = share > 2u ? share : 2u;
+  A.dynbase = A.rbeg + A.nstat * nwarps;
   k_stream<ADA><<<grid, 32 * kSWarps, 0, st>>>(A);
 }
 void launch_stream(const StepArgs& A, cudaStream_t st) {
