@@ -315,3 +315,33 @@ def test_split_rounds_and_resident_mode(gpu, oracle_mod, ipl):
     per launch (the bench's resident-state mode): sampled replicas, both halves and their borders, against the oracle."""
     _full_size_sampled(gpu, oracle_mod, W.config5(n_seeds=8192, n_requests=640),
                        [0, 1, 2047, 4094, 4095, 4096, 4097, 6000, 8190, 8191], ipl=ipl)
+
+
+# ------------------------------------------------------------------------------------------ streaming kernel, randomised
+
+@pytest.mark.parametrize("seed", range(8))
+def test_stream_path_randomised(gpu, oracle_mod, seed):
+    """The streaming kernel's own territory (FCFS / BOOST, paper's signal and quantiser): random batch cap, token
+    budget, chunk, KV size, bin size, guard on / off, hysteresis on / off, bursty arrivals that grow windows to a
+    few hundred requests (several chunks, parked-request merges, walk stops, evictions), 1 or 3 iterations per launch."""
+    rng = np.random.default_rng([77, seed])
+    n, NT = 700, 3
+    P = rng.integers(1, 400, (NT, n)); D = rng.integers(1, 120, (NT, n))
+    gaps = rng.exponential(2500, (NT, n)) * rng.choice([0.05, 1.0, 3.0], (NT, n), p=[0.3, 0.5, 0.2])
+    a = np.cumsum(gaps, axis=1).astype(np.int64)
+    R = 12
+    rep = W.make_replicas(R, trace_id=np.arange(R) % NT, policy=rng.choice([W.POLICY_FCFS, W.POLICY_BOOST], R),
+                          guard=rng.integers(0, 2, R), hysteresis_us=rng.choice([0, 100_000], R),
+                          gamma=rng.choice([0.05, 0.3, 2.0, 50.0], R))
+    blk = 16
+    kvb = int(rng.integers(60, 400))
+    D = np.minimum(D, np.maximum(1, kvb * blk - P))
+    sim = dict(kv_blocks=kvb, queue_cap=int(rng.choice([400, 700])), max_batch=int(rng.choice([8, 48, 256])),
+               chunk_tokens=int(rng.choice([16, 64, 512])), token_budget=int(rng.choice([64, 256, 1024])),
+               bin_tokens=int(rng.choice([16, 64, 256])), preempt_mode=int(rng.integers(0, 3)),
+               swap_pool_blocks=int(rng.integers(0, 200)))
+    wl = W.custom(a, P, D, sim, rep)
+    g, o = _pair(gpu, oracle_mod, wl, ipl=int(rng.choice([1, 3])))
+    g.run(); o.run()
+    _assert_same(g, o, f"randomised stream case {seed}: {sim}")
+    assert max(s["peak_active"] for s in o.stats()) > 64
