@@ -440,22 +440,46 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           const uint32_t sig1 = r0.P + r1.d + 1u;                      // signal after this token
           const bool okl = (fl & (F_LOCK_MASK_LOW)) == (F_RESIDENT | F_ADMITNOW | F_EMITPREV) && r1.cached + 2u == sig1 &&
                            r1.d + 1u != r0.D && sig1 != (k << (fl >> F_LOCK_SHIFT));
-          if (__all_sync(kFull, okl || !valid)) {
-            const uint32_t nv = __popc(cv);
-            const uint32_t totf = __reduce_add_sync(kFull, valid ? (r1.cached + 1u + blk_m1) >> blk_sh : 0u);
+          // ... optionally followed, when nothing is parked, by steadily waiting requests (not resident, nothing to
+          // finalise) whose first one is turned away -- on KV ("newblocked": the walk goes on over residents only,
+          // of which this chunk has none left) or because the batch / token budget is used up (the walk stops)
+          const bool okw = !okl && (fl & ~F_SWAPPED) == F_KLASS1;
+          const uint32_t decm = __ballot_sync(kFull, valid && okl);
+          const uint32_t wm = pend ? 0u : __ballot_sync(kFull, valid && okw);
+          if ((decm | wm) == cv && (wm == 0u || decm < (wm & (0u - wm)))) {    // (decoders first)
+            const uint32_t nv = __popc(decm);
+            const uint32_t totf = __reduce_add_sync(kFull, (valid && okl) ? (r1.cached + 1u + blk_m1) >> blk_sh : 0u);
             if (crank + nv <= M && carryW + nv <= Tb && carryC + totf <= B) {
-              const uint32_t np = outpos + __popc(cv & ltmask);
-              if (valid) {
-                if (np != c * 32u + (uint32_t)lane)
-                  __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
-                __stcg(reinterpret_cast<int4*>(gE1 + np),
-                       make_int4((int)r1.id, (int)(r1.d + 1u), (int)(r1.cached + 1u), (int)fl));
-                const uint64_t h = (uint64_t)(((r1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu)) * 3ull;
-                evl += (uint32_t)h; evu += (uint32_t)(h >> 32);
-                de += 0x10001u; ps += 0x10000u;
+              uint32_t nmode = 0;
+              if (wm) {
+                const uint32_t tokb = carryW + nv, cbw = crank + nv;
+                nmode = 2u;
+                if (cbw < M && tokb < Tb) {                            // would it fit?  want = min(c, rem, T - tok)
+                  const uint32_t rem = r0.P + r1.d - r1.cached;
+                  uint32_t wnt = rem < cc ? rem : cc;
+                  wnt = wnt < Tb - tokb ? wnt : Tb - tokb;
+                  const uint32_t footw = __shfl_sync(kFull, (r1.cached + wnt + blk_m1) >> blk_sh, __ffs(wm) - 1);
+                  nmode = (carryC + totf + footw > B) ? 1u : 3u;       // 3: it is admitted -> general path
+                }
               }
-              crank += nv; carryW += nv; carryC += totf; outpos += nv;
-              continue;
+              if (nmode != 3u) {
+                const uint32_t np = outpos + __popc(cv & ltmask);
+                const bool moved = np != c * 32u + (uint32_t)lane;
+                if (valid && moved) __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
+                if (valid && okl) {
+                  __stcg(reinterpret_cast<int4*>(gE1 + np),
+                         make_int4((int)r1.id, (int)(r1.d + 1u), (int)(r1.cached + 1u), (int)fl));
+                  const uint64_t h = (uint64_t)(((r1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu)) * 3ull;
+                  evl += (uint32_t)h; evu += (uint32_t)(h >> 32);
+                  de += 0x10001u; ps += 0x10000u;
+                } else if (valid && moved) {
+                  __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
+                }
+                carryW += nv; carryC += totf; carryN = crank + nv;     // (carryN: the turned-away request's rank)
+                crank += __popc(cv); outpos += __popc(cv);
+                mode = nmode;
+                continue;
+              }
             }
           }
         }
