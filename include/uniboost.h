@@ -154,6 +154,13 @@ int  ub_tbt_hist(ub_sim*, uint32_t replica, uint32_t* hist);
 int  ub_debug_get_state(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t* id, uint32_t* d,
                         uint32_t* cached, uint32_t* flags, int64_t* clock_us);
 
+/* Kernel-level parity (SURVEY.md Sec. 4 tier T1): the (class, key) the device assigns to every request of a replica's
+ * window as it stands now, i.e. as the NEXT iteration would score the requests already in the window (a1, M3-M5, M14)
+ * -- computed by the same device function the team kernels use.  id, klass: host [queue_cap] u32; key_us: host
+ * [queue_cap] i64 (microseconds, or tokens for SRPT / LAS / SJF / SPF); each nullable; *n_active receives the count.
+ * Entries come in stored (last priority) order.  Synchronises. */
+int  ub_debug_keys(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us);
+
 /* Timing of the step kernel launches issued by the LAST ub_step / ub_run call, measured with CUDA events on
  * the borrowed stream: total milliseconds and launch count.  Synchronises. */
 int  ub_last_step_timing(ub_sim*, float* kernel_ms, uint32_t* launches);

@@ -2,7 +2,7 @@
 // the host-side fp64 build of the fixed-point boost table (Eq. 2, rule M4) and the launch loops.
 // Every step of the scheduling path itself runs in the kernels of ub_step.cu / ub_aux.cu.
 #include "../../include/uniboost.h"
-#include "ub_internal.cuh"
+#include "ub_device.cuh"
 
 #include <math.h>
 #include <stdlib.h>
@@ -633,6 +633,47 @@ int ub_tbt_hist(ub_sim* s, uint32_t r, uint32_t* hist) {
   if (set_dev(s)) return UB_ECUDA;
   CK(cudaMemcpyAsync(hist, s->d_hist + (size_t)r * kTbtBins, kTbtBins * 4, cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
+  return UB_OK;
+}
+
+__global__ void k_debug_keys(SimDev s, uint32_t r, uint32_t n, uint32_t* id, unsigned long long* okey) {
+  const RepPar par = s.par[r];
+  const int64_t* lut = s.lut + par.lut_off + (size_t)s.hdr[r].level * 64u;
+  const int64_t* tfirst = s.t_first + (size_t)r * s.N;
+  for (uint32_t p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += gridDim.x * blockDim.x) {
+    const Rec0 q0 = s.E0[(size_t)r * s.Q + p];
+    const Rec1 q1 = s.E1[(size_t)r * s.Q + p];
+    id[p] = q1.id;
+    okey[p] = okey_of(s, par, lut, tfirst, q0, q1);
+  }
+}
+
+int ub_debug_keys(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us) {
+  if (!s || r >= s->cfg.n_replicas) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  Hdr h;
+  CK(cudaMemcpyAsync(&h, s->d_hdr + r, sizeof(Hdr), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  const uint32_t n = h.n_active;
+  if (n_active) *n_active = n;
+  if (!n) return UB_OK;
+  uint32_t* d_id = nullptr; unsigned long long* d_key = nullptr;
+  int rc = UB_OK;
+  if ((rc = dmalloc(&d_id, n)) || (rc = dmalloc(&d_key, n))) { cudaFree(d_id); cudaFree(d_key); return rc; }
+  k_debug_keys<<<(n + 127) / 128, 128, 0, s->stream>>>(s->dev, r, n, d_id, d_key);
+  std::vector<uint32_t> hid(n); std::vector<unsigned long long> hk(n);
+  cudaError_t e = cudaMemcpyAsync(hid.data(), d_id, n * 4, cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(hk.data(), d_key, n * 8, cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(d_id); cudaFree(d_key);
+  if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  for (uint32_t i = 0; i < n; i++) {
+    if (id) id[i] = hid[i];
+    if (klass) klass[i] = (uint32_t)(hk[i] >> 63);
+    if (key_us) key_us[i] = (int64_t)(hk[i] & ~(1ull << 63)) - kKeyBias;
+  }
   return UB_OK;
 }
 

@@ -219,25 +219,8 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
       const uint32_t pos = c * TH + tid;
       key[c] = ~0ull;
       if (pos < n) {
-        const uint32_t sig = signal_of(par, r0[c].P, r0[c].D, r1[c].d);
-        const uint32_t bin = bin_of(par, s.k, sig);
-        int64_t kv;
-        if (par.policy == 0) kv = r0[c].a;
-        else if (par.policy == 1) kv = (int64_t)(r0[c].D - r1[c].d);
-        else if (par.policy == 3) kv = (int64_t)sig;
-        else if (par.policy == 4) kv = (int64_t)r0[c].D;                               // SJF, perfect lengths
-        else if (par.policy == 5) kv = (int64_t)r0[c].P;                               // SPF
-        else if (par.policy == 6) {                                                    // DistBoost (M14), Eq. 3-4
-          if (r1[c].d >= 1u) kv = __ldcg(g_tfirst + r1[c].id);
-          else { const uint32_t pb = bin_of(par, s.k, r0[c].P); kv = r0[c].a - __ldg(lut + (pb < par.lut_nb ? pb : par.lut_nb - 1)); }
-        }
-        else kv = r0[c].a - __ldg(lut + (bin < par.lut_nb ? bin : par.lut_nb - 1));   // pi = a - b
-        const bool res = (r1[c].flags & F_RESIDENT) != 0;
-        if (res && (par.policy == 0 || par.policy == 2)) kv -= par.delta;             // Eq. 7 as a bias
-        const uint32_t lockp1 = r1[c].flags >> F_LOCK_SHIFT;
-        uint64_t klass = (par.guard && res && lockp1 == bin + 1u) ? 0ull : 1ull;
-        if (par.policy == 6) klass = r1[c].d >= 1u ? 0ull : 1ull;                     // decode batch first, Eq. 5-6
-        key[c] = (klass << 63) | (uint64_t)(kv + kKeyBias);
+        key[c] = okey_of(s, par, lut, g_tfirst, r0[c], r1[c]);
+        const uint64_t klass = key[c] >> 63;
         const uint32_t dirty = (r1[c].flags & F_DIRTY) ? 1u : 0u;
         n_dirty += dirty;
         KeyRec kr; kr.okey = key[c]; kr.id = r1[c].id; kr.aux = dirty;

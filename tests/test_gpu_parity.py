@@ -345,3 +345,28 @@ def test_stream_path_randomised(gpu, oracle_mod, seed):
     g.run(); o.run()
     _assert_same(g, o, f"randomised stream case {seed}: {sim}")
     assert max(s["peak_active"] for s in o.stats()) > 64
+
+
+# ------------------------------------------------------------------------------------------ kernel-level parity: a1 score
+
+@pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS, W.POLICY_SJF,
+                                    W.POLICY_SPF, W.POLICY_DISTBOOST])
+def test_score_kernel_keys_match_oracle(gpu, oracle_mod, policy):
+    """SURVEY.md Sec. 4 tier T1: before every iteration the (class, key) the device assigns to each request of the
+    window (ub_debug_keys, the team kernels' own scoring function) equals what the oracle scores in that iteration."""
+    wl = pressure_workload(6, n=140, kv_blocks=48, policy=policy, preempt=W.PRE_AUTO, swap_pool_blocks=20,
+                           guard=1 if policy == W.POLICY_BOOST else 0, gamma=0.3, bin_tokens=32)
+    g, o = _pair(gpu, oracle_mod, wl)
+    checked = 0
+    for it in range(1500):
+        ids, kl, ky = g.debug_keys(0)
+        info, rows = o.step_replica(0)
+        g.step(1)
+        if not info["executed"]:
+            break
+        want = {r["id"]: (r["klass"], r["key"]) for r in rows}
+        for i, c, k in zip(ids, kl, ky):
+            assert (int(c), int(k)) == want[int(i)], f"iteration {it} request {i}"
+        checked += len(ids)
+        assert g.digest()[0] == o.digest()[0]
+    assert checked > 5000
