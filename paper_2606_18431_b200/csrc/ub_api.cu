@@ -325,6 +325,13 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
       launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, i ? s->aux[i - 1] : s->stream);
     }
     n_iters -= k; nl++;
+    // what k_stream queued for the team kernels runs at the end of the call (all owed iterations at once); with
+    // gamma-Ada after every round, because UPDATEGAMMA sits between the iterations
+    if (ada || n_iters == 0)
+      for (uint32_t i = 0; i < ns; i++) {
+        const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
+        flush_slow(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, rb, re, i ? s->aux[i - 1] : s->stream);
+      }
   }
   if (ns > 1) {
     for (uint32_t i = 1; i < ns; i++) {

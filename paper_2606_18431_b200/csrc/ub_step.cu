@@ -699,27 +699,43 @@ int step_configure(uint32_t) {
   return (int)e;
 }
 
-// One scheduler round (`iters` iterations of every live replica): the streaming kernel (ub_stream.cu) visits every
-// replica and queues what it does not handle (SRPT / LAS keys, test-only modes, re-key bursts) for the team kernels:
-// L list, M list, S list, then the overflow list.
-void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 cudaStream_t st) {
-  StepArgs A;
-  A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend;
+// One scheduler round (`iters` iterations of every live replica) is ONE launch: the streaming kernel (ub_stream.cu)
+// visits every replica.  What it does not handle itself (SRPT / LAS / SJF / SPF / DistBoost keys, test-only modes,
+// re-key bursts) it queues ONCE for the team kernels and from then on only counts the iterations that replica owes
+// (Hdr::todo); replicas are independent, so the owed iterations are run later, all at once, by flush_slow(): L list,
+// M list, S list, then the overflow list.  (The 8-warp L kernel needs a whole SM per CTA; launched after every round
+// it stalled the stream of k_stream launches by 14 % although its list is empty in config 5.)
+static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg,
+                      uint32_t rend) {
+  A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend; A.nstat = A.dynbase = 0;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
   if (s.all_stream) A.thrS = A.thrM = 0;                                        // (windows are never empty when queued)
-  cudaMemsetAsync(count, 0, 5 * sizeof(uint32_t), st);                          // this round's lists and ticket counter
+}
+
+void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
+                 cudaStream_t st) {
+  StepArgs A;
+  make_args(A, s, list, count, iters, rbeg, rend);
+  cudaMemsetAsync(count + 4, 0, sizeof(uint32_t), st);                          // this round's ticket counter
   launch_stream(A, st);
+}
+
+// Runs the iterations owed by the queued replicas and empties the lists.
+void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, cudaStream_t st) {
+  StepArgs A;
+  make_args(A, s, list, count, 1, rbeg, rend);
   const uint32_t R = rend - rbeg;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;
   const uint32_t nS = (R + kTeamsS - 1) / kTeamsS, gS = nS < 148u * 10 ? nS : 148u * 10;
   k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 2u, 0xFFFFFFFFu);
-  if (s.all_stream) return;                      // nothing can be queued for the smaller teams
-  k_step<4, kEM, 1><<<gM, 128, TeamSmem<4, kEM>::BYTES, st>>>(A, 1u, 0xFFFFFFFFu);
-  k_step<1, kES, kTeamsS><<<gS, 32 * kTeamsS, kTeamsS * TeamSmem<1, kES>::BYTES, st>>>(A, 0u, 0xFFFFFFFFu);
-  k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 3u, 0xFFFFFFFFu);
+  if (!s.all_stream) {                           // (else nothing can be queued for the smaller teams)
+    k_step<4, kEM, 1><<<gM, 128, TeamSmem<4, kEM>::BYTES, st>>>(A, 1u, 0xFFFFFFFFu);
+    k_step<1, kES, kTeamsS><<<gS, 32 * kTeamsS, kTeamsS * TeamSmem<1, kES>::BYTES, st>>>(A, 0u, 0xFFFFFFFFu);
+    k_step<8, kEL, 1><<<gL, 256, TeamSmem<8, kEL>::BYTES, st>>>(A, 3u, 0xFFFFFFFFu);
+  }
+  cudaMemsetAsync(count, 0, 4 * sizeof(uint32_t), st);                          // the lists are empty again
 }
 
 }  // namespace ub

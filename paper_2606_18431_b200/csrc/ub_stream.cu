@@ -125,6 +125,14 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 #define UB_DELTA (reinterpret_cast<const RepPar*>(X.par[parity])->delta)
     uint32_t n = (uint32_t)sh[13];
     if (n == 0 && (int64_t)sh[2] == kNever) continue;                 // finished its trace
+    {
+      // a replica queued for the team kernels owes them its iterations until they have run (Hdr::todo, flush_slow)
+      const uint32_t todo = (uint32_t)(sh[17] >> 32);
+      if (todo) {
+        if (lane == 0) reinterpret_cast<uint32_t*>(UB_H64 + 17)[1] = todo + A.iters;
+        continue;
+      }
+    }
     uint32_t nd = (uint32_t)sh[18];                                   // entries of the dirty list
     const uint32_t iters = A.iters;
     const RepPar par = *reinterpret_cast<const RepPar*>(X.par[parity]);
@@ -683,7 +691,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 
     // ---------------- not handled here: queue the replica for the team kernels of this round
     if (slow && lane == 0) {
-      if (it > 0) reinterpret_cast<uint32_t*>(UB_H64 + 17)[1] = iters - it;       // iterations still to do
+      reinterpret_cast<uint32_t*>(UB_H64 + 17)[1] = iters - it;                 // iterations it owes the team kernels
       push_list(A, s.all_stream ? 2u : (wsize <= A.thrS ? 0u : (wsize <= A.thrM ? 1u : 2u)), r);
     }
   }
