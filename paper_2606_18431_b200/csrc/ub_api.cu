@@ -36,6 +36,7 @@ struct ub_sim {
   cudaEvent_t ev0, ev1;
   cudaStream_t aux[3]; cudaEvent_t ev_fork, ev_join[3];   // extra streams: the parts of a round overlap their tails
   uint32_t nsplit;
+  uint32_t round_no;            // launches alternate between two ticket counters
   float last_ms; uint32_t last_launches;
 };
 
@@ -322,9 +323,9 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
     for (uint32_t i = 0; i < ns; i++) {
       const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
       if (ada) launch_gamma_ada(s->dev, rb, re, i ? s->aux[i - 1] : s->stream);
-      launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, i ? s->aux[i - 1] : s->stream);
+      launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, s->round_no, i ? s->aux[i - 1] : s->stream);
     }
-    n_iters -= k; nl++;
+    n_iters -= k; nl++; s->round_no++;
     // what k_stream queued for the team kernels runs at the end of the call (all owed iterations at once); with
     // gamma-Ada after every round, because UPDATEGAMMA sits between the iterations
     if (ada || n_iters == 0)

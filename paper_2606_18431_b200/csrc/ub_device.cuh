@@ -101,6 +101,7 @@ struct StepArgs {
   SimDev s;
   uint32_t* list; uint32_t* count;
   uint32_t iters;
+  uint32_t tick;                // which of the two ticket counters (count[4], count[6]) this launch draws from
   uint32_t nstat, dynbase;      // k_stream work distribution (set by launch_stream): static replicas per warp, first ticket
   uint32_t rbeg, rend;          // replicas [rbeg, rend) belong to this launch (a round may be split over two streams)
   uint32_t thrS, thrM;          // window size up to which a replica is queued for the S / M kernel

@@ -91,7 +91,7 @@ struct SimDev {                 // kernel argument (by value)
 
 // kernels (ub_step.cu, ub_aux.cu)
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 cudaStream_t st);
+                 uint32_t tick, cudaStream_t st);
 void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, cudaStream_t st);
 void launch_stream(const struct StepArgs& A, cudaStream_t st);    // ub_stream.cu
 void launch_gamma_ada(const SimDev& s, uint32_t rbeg, uint32_t rend, cudaStream_t st);   // ub_aux.cu

@@ -707,7 +707,7 @@ int step_configure(uint32_t) {
 // it stalled the stream of k_stream launches by 14 % although its list is empty in config 5.)
 static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg,
                       uint32_t rend) {
-  A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend; A.nstat = A.dynbase = 0;
+  A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend; A.nstat = A.dynbase = A.tick = 0;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
@@ -715,10 +715,10 @@ static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* co
 }
 
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 cudaStream_t st) {
+                 uint32_t tick, cudaStream_t st) {
   StepArgs A;
   make_args(A, s, list, count, iters, rbeg, rend);
-  cudaMemsetAsync(count + 4, 0, sizeof(uint32_t), st);                          // this round's ticket counter
+  A.tick = tick & 1u;
   launch_stream(A, st);
 }
 

@@ -105,18 +105,20 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 
   // Work distribution: windows differ by two orders of magnitude.  A warp takes its first `nstat` replicas by static
   // striding (3/4 of an even share); the rest are handed out dynamically: each is the next value of a global ticket
-  // counter (count[4], zeroed per round), requested one replica ahead so that the atomic's latency is never waited for.
+  // counter (count[4] / count[6] alternately, each zeroed by the launch before), requested one replica ahead so that the atomic's latency is never waited for.
 #define UB_GW (A.rbeg + blockIdx.x * kSWarps + (threadIdx.x >> 5))
   uint32_t r = UB_GW, rn = UB_GW + nwarps;
   uint32_t taken = 2, ticket = 0;
   uint32_t parity = 0;
   prefetch_replica(r, 0);
+  // (the ticket counter of the NEXT launch is zeroed here: launches of one part alternate between the two)
+  if (blockIdx.x == 0 && threadIdx.x == 0) A.count[4 + 2 * (A.tick ^ 1u)] = 0u;
   for (; r < A.rend; r = rn, rn = (taken < A.nstat ? UB_GW + taken * nwarps : __shfl_sync(kFull, ticket, 0) + A.dynbase), taken++,
                   parity ^= 1u) {
     cp_wait<0>();
     __syncwarp();
     prefetch_replica(rn, parity ^ 1u);
-    if (taken >= A.nstat && lane == 0) ticket = atomicAdd(A.count + 4, 1u);
+    if (taken >= A.nstat && lane == 0) ticket = atomicAdd(A.count + 4 + 2 * A.tick, 1u);
     const unsigned long long* sh = reinterpret_cast<const unsigned long long*>(X.hdr[parity]);
     // (addresses and per-replica scalars that are needed rarely are re-derived where they are used instead of
     // living in registers across the chunk loop)
