@@ -6,8 +6,8 @@ requests, 50/50 chat/reasoning mix, Poisson arrivals at 95 % load, KV capacity 1
 BOOST gamma = 0.3, swap-vs-recompute preemption; seeded synthetic traces (workloads.config5).
 
 A "step" is one ub_step(h, ITERS) call: every replica advances ITERS scheduler iterations, each iteration one
-launch of the streaming step kernel ub::k_stream (all of a0..a5: the replica's window goes HBM -> SM -> HBM once)
-followed by the four team-kernel launches that take what it queued (none in this config).  Before the timed
+launch of the streaming step kernel ub::k_stream per half of the replicas (all of a0..a5: the replica's window goes
+HBM -> SM -> HBM once); what it queues for the team kernels (nothing in this config) runs once per ub_step call.  Before the timed
 region every replica is advanced SPINUP iterations (not timed, default 65536 = the middle of the ~1.4e5
 iterations a config-5 replica runs) so that the queues are in their loaded regime.  The timed region is K steps on
 the device (CUDA events, barrier + synchronize on both sides, max over ranks).  The windows read per launch
@@ -35,7 +35,7 @@ from paper_2606_18431_b200 import workloads as W  # noqa: E402
 
 RESIDENT_IPL = 16
 KERNELS_PER_ROUND = 2                # a round = two halves on two streams, one ub::k_stream launch each (team kernels run once per ub_step)
-TRAFFIC_BYTES_PER_LAUNCH = 463.4e6   # dram read+write bytes of the two ub::k_stream launches of one round, profiles/r01e_stream.md
+TRAFFIC_BYTES_PER_LAUNCH = 463.3e6   # dram read+write bytes of the two ub::k_stream launches of one round, profiles/r01f_stream.md
 ALG_BYTES_PER_REQUEST_STEP = 40      # read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
 METRIC = "request-steps scheduled/sec"
 UNIT = "request-steps/s"
@@ -274,7 +274,7 @@ def main():
                          "request_steps_per_launch": (rs2 - rs1) / max(1, rounds),
                          "avg_launch_ms": ms / max(1, rounds),
                          "note": "a round = every live replica advanced one iteration = two overlapping k_stream launches "
-                                 "(one half of the replicas each, on two streams) + two (empty here) team-kernel launches; "
+                                 "(one half of the replicas each, on two streams); the team kernels run once per ub_step; "
                                  "avg_launch_ms, request_steps_per_launch and traffic are per round; traffic = dram "
                                  "read+write bytes of the round's k_stream launches from profiles/ (ncu --set full)"},
             "e2e": {"value": rs_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
