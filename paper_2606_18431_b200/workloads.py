@@ -292,6 +292,37 @@ def starvation(n_seeds: int = 1, n_requests: int = 2000, load: float = 0.99) -> 
                     np.arange(n_seeds))
 
 
+def routed_cluster(n_replicas: int = 8, n_requests_total: int = 6000, dispatch: str = "round_robin", load: float = 0.9,
+                   seed: int = 0, kv_blocks: int = 4096):
+    """Global dispatch in front of per-replica scheduling (Tables 9-10: "the routing policy is
+    exogenous", the part that keeps replicas independent): ONE global Poisson stream at
+    load x n_replicas x lambda_cap (50/50 chat / reasoning mix) is split over the replicas by a router that does not
+    look at replica state -- "round_robin" (request i -> replica i mod R) or "random" (seeded uniform choice).
+    Join-the-shortest-queue looks at queue lengths at arrival time and would couple the replicas: not built.
+    Returns (workload, traces) with ragged per-replica request counts (traces[3])."""
+    if dispatch not in ("round_robin", "random"):
+        raise ValueError("dispatch must be 'round_robin' or 'random'")
+    R, T = int(n_replicas), int(n_requests_total)
+    rng = np.random.default_rng([7, seed])
+    Pc, Dc = _chat_lengths(rng, T)
+    Pr, Dr = _reasoning_lengths(rng, T)
+    is_chat = rng.random(T) < 0.5
+    P = np.where(is_chat, Pc, Pr); D = _fit_kv(P, np.where(is_chat, Dc, Dr), kv_blocks * 16)
+    sim0 = _sim(R, R, 1, 2048, kv_blocks, preempt_mode=PRE_AUTO, swap_pool_blocks=kv_blocks)
+    arr = _poisson_arrivals(rng, T, load * R * capacity_rate(P, D, sim0))
+    dest = (np.arange(T) % R) if dispatch == "round_robin" else rng.integers(0, R, T)
+    counts = np.bincount(dest, minlength=R)
+    N = int(max(1, counts.max()))
+    a = np.zeros((R, N), np.int64); p = np.ones((R, N), np.int32); d = np.ones((R, N), np.int32)
+    for r in range(R):
+        sel = np.nonzero(dest == r)[0]                  # arrival order is kept inside a replica
+        a[r, :len(sel)], p[r, :len(sel)], d[r, :len(sel)] = arr[sel], P[sel], D[sel]
+    sim = dict(sim0, max_requests=N, queue_cap=min(N, 2048))
+    wl = Workload(f"routed cluster: {R} replicas, {T} requests, {dispatch}", 7, sim, make_replicas(R),
+                  lambda s_: (a[s_], p[s_], d[s_]), np.arange(R))
+    return wl, (a, p, d, counts.astype(np.uint32)), (arr, P.astype(np.int32), D.astype(np.int32), dest)
+
+
 def by_id(config_id: int, **kw) -> Workload:
     return {1: config1, 2: config2, 3: config3, 4: config4, 5: config5, 6: starvation}[config_id](**kw)
 
