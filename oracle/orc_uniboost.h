@@ -15,7 +15,9 @@
  * and hysteresis (Eq. 7), Sec. 3.3 MemGuard (PAPER.md:198-215,
  * Eq. 8), on top of the per-iteration cost model that BASELINE.json states
  * (config 1 and config 3).  Where the paper is silent the readings are the
- * ones listed in DESIGN.md Sec. 3 (model rules M1..M12, readings G1..G21).
+ * ones listed in DESIGN.md Sec. 3 (model rules M1..M14, readings G1..G24; M13 =
+ * gamma-Ada, Eq. 9 / UPDATEGAMMA; M14 = DistBoost,
+ * Eq. 3-6; baselines SJF / SPF as static keys).
  * The method is a policy (a heuristic driven by a priority rule), not a
  * faster route to a closed form, so the oracle is the algorithm written out
  * step by step in the paper's order: score every active request, sort,
@@ -32,7 +34,12 @@
  *   tiny traces, Eq. 6 arg-min subset, MemGuard logarithmic
  *   bound, Lemma A.1 boost bound,
  *   percentile definition vs numpy inverted_cdf, a hand-worked
- *   schedule (tests/golden/hand_trace_*.txt).
+ *   schedules (tests/golden/hand_traces.{md,json}); Smith's rule brute force
+ *   (SJF / SPF); Lindley recursion and the Eq. 3-6 queue structure (DistBoost);
+ *   tests/test_gamma_ada_pins.py: Eq. 9 on an exactly exponential tail, the
+ *   log-spaced grid, no update == static gamma, the update rule re-derived every
+ *   iteration; tests/test_reductions.py: numpy inverted_cdf at per-mille points
+ *   and plain counts (percentile curve, SLO attainment).
  * Parity UNPINNED: the paper's latency tables (Tables 2-10) -- they need real
  * GPUs, model weights and datasets that are not available.
  */
