@@ -21,13 +21,13 @@ struct ub_sim {
   cudaStream_t stream;
   bool have_trace, have_reps;
   // owned device memory
-  Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; RepPar* d_par; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
+  Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
   int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
   uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([5] = finished replicas)
   int64_t* d_ada_ring; AdaState* d_ada_state; int64_t* d_ada_grid;   // gamma-Ada (M13), null when off
   std::vector<int64_t> h_ada_grid;
-  uint16_t* d_dlist; uint2* d_evbuf;     // dirty lists [R][kDirtyMax]; per-iteration event scratch [R][min(M,Q)]
+  uint2* d_evbuf;                        // per-iteration event scratch [R][min(M,Q)]
   unsigned long long* h_word;            // pinned
   std::vector<uint32_t> h_nreq, h_maxsig;
   std::vector<ub_replica> h_reps;
@@ -91,11 +91,10 @@ int ub_create(const ub_config* c, ub_sim** out) {
   const size_t R = c->n_replicas, Q = c->queue_cap, N = c->max_requests, NT = c->n_traces;
   int rc = UB_OK;
   if ((rc = dmalloc(&s->d_E0, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_E1, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_hdr, R)) ||
-      (rc = dmalloc(&s->d_par, R)) || (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
+      (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
       (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 4 * kMaxSplit * R)) || (rc = dmalloc(&s->d_count, 8 * kMaxSplit)) ||
-      (rc = dmalloc(&s->d_dlist, R * kDirtyMax)) ||
       (rc = dmalloc(&s->d_evbuf, R * (size_t)(c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap)))) {
     ub_destroy(s);
     return rc;
@@ -122,8 +121,8 @@ int ub_create(const ub_config* c, ub_sim** out) {
   d.B = c->kv_blocks; d.blk = c->block_tokens; d.M = c->max_batch; d.c = c->chunk_tokens; d.T = c->token_budget;
   d.preempt_mode = c->preempt_mode; d.swap_ns = c->swap_ns_per_block; d.swap_pool = c->swap_pool_blocks;
   d.k = c->bin_tokens; d.c0 = c->c0_us; d.c_pf = c->c_prefill_tok_us; d.c_dec = c->c_decode_seq_us;
-  d.E0 = s->d_E0; d.E1 = s->d_E1; d.hdr = s->d_hdr; d.par = s->d_par; d.n_req = s->d_nreq;
-  d.dlist = s->d_dlist; d.evbuf = s->d_evbuf; d.evcap = c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap;
+  d.E0 = s->d_E0; d.E1 = s->d_E1; d.hdr = s->d_hdr; d.n_req = s->d_nreq;
+  d.evbuf = s->d_evbuf; d.evcap = c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap;
   d.t_first = s->d_tfirst; d.t_last = s->d_tlast; d.n_evict = s->d_ne; d.n_evict_unf = s->d_neu; d.hist = s->d_hist;
   *out = s;
   return UB_OK;
@@ -133,10 +132,10 @@ void ub_destroy(ub_sim* s) {
   if (!s) return;
   cudaSetDevice(s->cfg.device);
   cudaStreamSynchronize(s->stream);
-  cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_par); cudaFree(s->d_TR);
+  cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_TR);
   cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
-  cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_dlist); cudaFree(s->d_evbuf);
+  cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_evbuf);
   cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);
   if (s->h_word) cudaFreeHost(s->h_word);
   if (s->ev0) cudaEventDestroy(s->ev0);
@@ -290,7 +289,8 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   int rc = dmalloc(&s->d_lut, s->h_lut.size()); if (rc) return rc;
   if (!s->h_lut.empty())
     CK(cudaMemcpyAsync(s->d_lut, s->h_lut.data(), s->h_lut.size() * 8, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->d_par, par.data(), R * sizeof(RepPar), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpy2DAsync(&s->d_hdr[0].par, sizeof(Hdr), par.data(), sizeof(RepPar), sizeof(RepPar), R,
+                       cudaMemcpyHostToDevice, s->stream));       // (parameters live inside the replica headers)
   s->dev.lut = s->d_lut;
   // reset the run state
   CK(cudaMemsetAsync(s->d_tfirst, 0xFF, R * N * 8, s->stream));     // -1
@@ -448,7 +448,7 @@ int ub_set_gamma_ada(ub_sim* s, const ub_gamma_ada* g, const uint8_t* adaptive) 
       s->h_lut.push_back(boost_table_entry(ada_grid_gamma(g, j), ldexp((double)c.bin_tokens, (int)b), c.tok_us));
   std::vector<AdaState> st(R);
   std::vector<RepPar> par(R);
-  CK(cudaMemcpy(par.data(), s->d_par, R * sizeof(RepPar), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy2D(par.data(), sizeof(RepPar), &s->d_hdr[0].par, sizeof(Hdr), sizeof(RepPar), R, cudaMemcpyDeviceToHost));
   for (size_t r = 0; r < R; r++) {
     memset(&st[r], 0, sizeof(AdaState));
     if (!adaptive[r]) continue;
@@ -467,7 +467,8 @@ int ub_set_gamma_ada(ub_sim* s, const ub_gamma_ada* g, const uint8_t* adaptive) 
       (rc = dmalloc(&s->d_ada_state, R)) || (rc = dmalloc(&s->d_ada_grid, (size_t)g->levels)))
     return rc;
   CK(cudaMemcpyAsync(s->d_lut, s->h_lut.data(), s->h_lut.size() * 8, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->d_par, par.data(), R * sizeof(RepPar), cudaMemcpyHostToDevice, s->stream));
+  CK(cudaMemcpy2DAsync(&s->d_hdr[0].par, sizeof(Hdr), par.data(), sizeof(RepPar), sizeof(RepPar), R,
+                       cudaMemcpyHostToDevice, s->stream));
   CK(cudaMemcpyAsync(s->d_ada_state, st.data(), R * sizeof(AdaState), cudaMemcpyHostToDevice, s->stream));
   CK(cudaMemcpyAsync(s->d_ada_grid, grid.data(), grid.size() * 8, cudaMemcpyHostToDevice, s->stream));
   CK(cudaMemsetAsync(s->d_ada_ring, 0, R * (size_t)g->window * 8, s->stream));
@@ -645,7 +646,7 @@ int ub_tbt_hist(ub_sim* s, uint32_t r, uint32_t* hist) {
 }
 
 __global__ void k_debug_keys(SimDev s, uint32_t r, uint32_t n, uint32_t* id, unsigned long long* okey) {
-  const RepPar par = s.par[r];
+  const RepPar par = s.hdr[r].par;
   const int64_t* lut = s.lut + par.lut_off + (size_t)s.hdr[r].level * 64u;
   const int64_t* tfirst = s.t_first + (size_t)r * s.N;
   for (uint32_t p = blockIdx.x * blockDim.x + threadIdx.x; p < n; p += gridDim.x * blockDim.x) {

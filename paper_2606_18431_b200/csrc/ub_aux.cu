@@ -42,9 +42,9 @@ void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, 
 __global__ void k_reset(SimDev s, uint32_t* count) {
   const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= s.R) return;
-  Hdr h;
-  memset(&h, 0, sizeof(h));
-  const uint32_t tr = s.par[r].trace_id;
+  Hdr h = s.hdr[r];                                 // (keeps the parameters ub_set_replicas wrote)
+  memset(&h, 0, offsetof(Hdr, par));
+  const uint32_t tr = h.par.trace_id;
   const bool empty = s.n_req[tr] == 0;
   h.a_next = empty ? kNever : s.TR[(size_t)tr * s.N].a;
   s.hdr[r] = h;
@@ -200,7 +200,7 @@ __global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out)
   __shared__ uint32_t wtot[kStatThreads / 32];
   const uint32_t r = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t tr = s.par[r].trace_id, nreq = s.n_req[tr];
+  const uint32_t tr = s.hdr[r].par.trace_id, nreq = s.n_req[tr];
   const Rec0* TR = s.TR + (size_t)tr * s.N;
   const int64_t* tf = s.t_first + (size_t)r * s.N;
   const int64_t* tl = s.t_last + (size_t)r * s.N;
@@ -263,7 +263,7 @@ struct CurveArgs { uint32_t which, n; uint32_t permille[16]; };
 __global__ void __launch_bounds__(kStatThreads) k_percentile_curve(SimDev s, CurveArgs c, int64_t* out) {
   __shared__ SelectSmem sm;
   const uint32_t r = blockIdx.x;
-  const uint32_t tr = s.par[r].trace_id, nreq = s.n_req[tr];
+  const uint32_t tr = s.hdr[r].par.trace_id, nreq = s.n_req[tr];
   const Rec0* TR = s.TR + (size_t)tr * s.N;
   const int64_t* src = (c.which == 0 ? s.t_first : s.t_last) + (size_t)r * s.N;
   const uint32_t* ne = s.n_evict + (size_t)r * s.N;
@@ -292,7 +292,7 @@ __global__ void __launch_bounds__(kStatThreads) k_slo_count(SimDev s, uint32_t w
                                                             uint32_t* out) {
   __shared__ uint32_t cnt[16];
   const uint32_t r = blockIdx.x;
-  const uint32_t tr = s.par[r].trace_id, nreq = s.n_req[tr];
+  const uint32_t tr = s.hdr[r].par.trace_id, nreq = s.n_req[tr];
   const Rec0* TR = s.TR + (size_t)tr * s.N;
   const int64_t* src = (which == 0 ? s.t_first : s.t_last) + (size_t)r * s.N;
   const uint32_t* ne = s.n_evict + (size_t)r * s.N;

@@ -5,10 +5,13 @@
 // arrays kept in PRIORITY ORDER of the last executed iteration (so the next iteration finds it nearly sorted):
 //   E0[r][Q] = { a: i64 arrival us, P: u32 prompt tokens, D: u32 hidden output tokens }   static per request
 //   E1[r][Q] = { id: u32, d: u32 tokens emitted, cached: u32 KV tokens held, flags: u32 } dynamic
-// plus one 160-byte header Hdr[r] (8-byte word i is addressed directly by the fast kernel: keep the order), the packed traces TR[trace][N] (same 16-byte record as E0), the
+// plus one 256-byte header Hdr[r] -- 160 bytes of state (8-byte word i is addressed directly by the streaming kernel:
+// keep the order), the replica's parameters and its dirty list, fetched together by one asynchronous copy --, the
+// packed traces TR[trace][N] (same 16-byte record as E0), the
 // per-request outputs t_first/t_last/n_evict/n_evict_unforced [R][N] and the TBT histogram [R][4352].
 #pragma once
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 namespace ub {
@@ -33,7 +36,16 @@ constexpr uint32_t kDirtyMax  = 32;        // entries of a replica's dirty list;
 struct __align__(16) Rec0 { int64_t a; uint32_t P; uint32_t D; };
 struct __align__(16) Rec1 { uint32_t id; uint32_t d; uint32_t cached; uint32_t flags; };
 
-struct __align__(16) Hdr {
+struct __align__(16) RepPar {   // per-replica parameters, read-only on the device (32 bytes: two cp.async pieces)
+  int64_t  delta;               // hysteresis_us
+  uint32_t trace_id;
+  uint32_t lut_off;             // offset of this replica's boost table in lut[]
+  uint32_t lut_nb;              // entries
+  uint8_t  policy, guard, signal_mode, quant_mode;
+  uint32_t pad[2];
+};
+struct __align__(16) Hdr {   // 256 bytes per replica: state (160), parameters (32), dirty list (64) -- one prefetch
+
   int64_t  t;                 // replica clock, us
   uint64_t H;                 // schedule digest (M12)
   int64_t  a_next;            // arrival of trace[next], kNever if exhausted
@@ -45,17 +57,12 @@ struct __align__(16) Hdr {
   uint32_t n_completed, evict_recompute, evict_swap, swapins;
   uint32_t done, todo, n_dirty, level;  // todo: iterations of this round still to do (hand-over between kernels);
                                         // level: gamma-Ada grid level (0 for a static replica), selects the boost table
+  uint32_t pad_state[2];
+  RepPar   par;               // per-replica parameters (read-only after ub_set_replicas)
+  uint16_t dl[kDirtyMax];     // window positions of the re-keyed ("dirty") requests
 };
-static_assert(sizeof(Hdr) == 160, "Hdr is 160 bytes");
+static_assert(sizeof(Hdr) == 256 && offsetof(Hdr, par) == 160, "Hdr: 160 bytes of state, then parameters and dirty list");
 
-struct __align__(16) RepPar {   // per-replica parameters, read-only on the device (32 bytes: two cp.async pieces)
-  int64_t  delta;               // hysteresis_us
-  uint32_t trace_id;
-  uint32_t lut_off;             // offset of this replica's boost table in lut[]
-  uint32_t lut_nb;              // entries
-  uint8_t  policy, guard, signal_mode, quant_mode;
-  uint32_t pad[2];
-};
 constexpr uint32_t kMaxSplit = 4;     // parts (streams) a scheduler round may be issued as
 constexpr uint32_t kWindowPad = 64;   // records allocated behind the last window (speculative chunk reads)
 
@@ -70,14 +77,12 @@ struct SimDev {                 // kernel argument (by value)
   int64_t  c0, c_pf, c_dec;
   // state
   Rec0* E0; Rec1* E1; Hdr* hdr;
-  const RepPar* par;
   const Rec0* TR;               // packed traces [NT][N]
   const uint32_t* n_req;        // [NT]
   const int64_t* lut;
   int64_t* t_first; int64_t* t_last;      // [R][N]
   uint32_t* n_evict; uint32_t* n_evict_unf;
   uint32_t* hist;               // [R][kTbtBins]
-  uint16_t* dlist;              // [R][kDirtyMax] window positions of the re-keyed ("dirty") requests
   uint2*    evbuf;              // [R][evcap] scratch: per-request events of one iteration that wait for t_end
   uint32_t  evcap;              // min(M, Q)
   // gamma-Ada (M13); ada_ring == nullptr when off

@@ -123,7 +123,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
   uint16_t* x_dl = x_idx + CAP;
   uint32_t* x_cnt = reinterpret_cast<uint32_t*>(x_dl + 32);
 
-  const RepPar par = s.par[r];
+  const RepPar par = s.hdr[r].par;
   const uint32_t nreq = s.n_req[par.trace_id];
   const Rec0* TR = s.TR + (size_t)par.trace_id * s.N;
   Rec0* gE0 = s.E0 + (size_t)r * s.Q;
@@ -603,7 +603,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
           *reinterpret_cast<int4*>(gE1 + np) = *reinterpret_cast<const int4*>(&r1[c]);
           if (r1[c].flags & F_DIRTY) {                       // the streaming kernel's dirty list (ub_stream.cu)
             const uint32_t slot = atomicAdd(&ts->ndirty, 1u);
-            if (slot < kDirtyMax) s.dlist[(size_t)r * kDirtyMax + slot] = (uint16_t)np;
+            if (slot < kDirtyMax) s.hdr[r].dl[slot] = (uint16_t)np;
           }
         }
         n_new += tot;

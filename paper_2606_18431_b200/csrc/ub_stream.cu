@@ -52,12 +52,10 @@ template <int N> __device__ __forceinline__ void cp_wait() { asm volatile("cp.as
 struct __align__(16) WarpBuf {             // per warp, 10 KB
   uint4 spec[2][2][64];                    // [parity][chunk 0 / 1][E0 records 0..31 | E1 records 32..63] of a replica
   uint4 ring[kRing][64];                   // chunks 2, 3, ... of the current replica
-  uint4 hdr[2][10];                        // Hdr (160 bytes)
-  uint4 par[2][2];                         // RepPar (32 bytes)
-  uint4 dl[2][4];                          // dirty list (32 x u16)
+  uint4 hdr[2][16];                        // Hdr (256 bytes: state, parameters, dirty list)
   uint4 sr0[32], sr1[32], skb[32];         // the dirty requests + arrivals of one iteration in key order;
 };                                         // skb = {key lo, key hi, bin, -}
-static_assert(sizeof(RepPar) == 32 && sizeof(Hdr) == 160, "cp.async copies these as 16-byte pieces");
+static_assert(sizeof(Hdr) == 256, "cp.async copies the header as sixteen 16-byte pieces");
 
 // a1 (M3-M5): sig = P + d; bin = Eq. 8 exponent; pi = a - b_gamma(w_hat) - delta if
 // resident (Eq. 7); key = class<<63 | (pi + 2^62); class 0 = MemGuard-locked resident.  All 32 lanes must call it.
@@ -91,10 +89,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   // header, parameters, dirty list and the first two chunks of replica rr -> stage `par` (one cp.async group)
   auto prefetch_replica = [&](const uint32_t rr, const uint32_t par) {
     if (rr < A.rend) {
-      if (lane < 10) cp16(&X.hdr[par][lane], reinterpret_cast<const uint4*>(s.hdr + rr) + lane);
-      else if (lane < 12) cp16(&X.par[par][lane - 10], reinterpret_cast<const uint4*>(s.par + rr) + (lane - 10));
-      else if (lane < 16)
-        cp16(&X.dl[par][lane - 12], reinterpret_cast<const uint4*>(s.dlist + (size_t)rr * kDirtyMax) + (lane - 12));
+      if (lane < 16) cp16(&X.hdr[par][lane], reinterpret_cast<const uint4*>(s.hdr + rr) + lane);
       const uint4* e0 = reinterpret_cast<const uint4*>(s.E0 + (size_t)rr * Q) + lane;
       const uint4* e1 = reinterpret_cast<const uint4*>(s.E1 + (size_t)rr * Q) + lane;
       cp16(&X.spec[par][0][lane], e0);        cp16(&X.spec[par][0][32 + lane], e1);
@@ -123,8 +118,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     // (addresses and per-replica scalars that are needed rarely are re-derived where they are used instead of
     // living in registers across the chunk loop)
 #define UB_H64 (reinterpret_cast<unsigned long long*>(s.hdr + r))
-#define UB_TR (s.TR + (size_t)reinterpret_cast<const RepPar*>(X.par[parity])->trace_id * s.N)
-#define UB_DELTA (reinterpret_cast<const RepPar*>(X.par[parity])->delta)
+#define UB_TR (s.TR + (size_t)reinterpret_cast<const Hdr*>(X.hdr[parity])->par.trace_id * s.N)
+#define UB_DELTA (reinterpret_cast<const Hdr*>(X.hdr[parity])->par.delta)
     uint32_t n = (uint32_t)sh[13];
     if (n == 0 && (int64_t)sh[2] == kNever) continue;                 // finished its trace
     {
@@ -137,7 +132,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     }
     uint32_t nd = (uint32_t)sh[18];                                   // entries of the dirty list
     const uint32_t iters = A.iters;
-    const RepPar par = *reinterpret_cast<const RepPar*>(X.par[parity]);
+    const RepPar par = reinterpret_cast<const Hdr*>(X.hdr[parity])->par;
     Rec0* gE0 = s.E0 + (size_t)r * Q;
     Rec1* gE1 = s.E1 + (size_t)r * Q;
     const bool isboost = par.policy == 2;
@@ -207,8 +202,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       if (m) {
         int4 v0 = make_int4(0, 0, 0, 0), v1 = make_int4(0, 0, 0, 0);
         if ((uint32_t)lane < nd) {
-          spos = it == 0 ? (uint32_t)reinterpret_cast<const uint16_t*>(X.dl[parity])[lane]
-                         : (uint32_t)__ldcg(s.dlist + (size_t)r * kDirtyMax + lane);
+          spos = it == 0 ? (uint32_t)reinterpret_cast<const Hdr*>(X.hdr[parity])->dl[lane]
+                         : (uint32_t)__ldcg(s.hdr[r].dl + lane);
           v0 = __ldcg(reinterpret_cast<const int4*>(gE0 + spos));
           v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + spos));
         } else if ((uint32_t)lane < m) {
@@ -390,7 +385,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const uint32_t dm = __ballot_sync(kFull, keep && dirty);
         if (dm) {                                                     // next iteration's dirty list
           const uint32_t slot = ndnew + __popc(dm & ltmask);
-          if (keep && dirty && slot < kDirtyMax) s.dlist[(size_t)r * kDirtyMax + slot] = (uint16_t)np;
+          if (keep && dirty && slot < kDirtyMax) s.hdr[r].dl[slot] = (uint16_t)np;
           ndnew += __popc(dm);
         }
         outpos += __popc(keepm);
@@ -597,7 +592,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           const uint32_t dm = __ballot_sync(kFull, victim && !(of & F_DIRTY));      // residency changed => dirty
           if (dm) {
             const uint32_t slot = ndnew + __popc(dm & ltmask);
-            if (victim && !(of & F_DIRTY) && slot < kDirtyMax) s.dlist[(size_t)r * kDirtyMax + slot] = (uint16_t)pos;
+            if (victim && !(of & F_DIRTY) && slot < kDirtyMax) s.hdr[r].dl[slot] = (uint16_t)pos;
             ndnew += __popc(dm);
           }
           behind += tot;
