@@ -35,7 +35,7 @@ from paper_2606_18431_b200 import workloads as W  # noqa: E402
 
 RESIDENT_IPL = 16
 KERNELS_PER_ROUND = 2                # a round = two halves on two streams, one ub::k_stream launch each (team kernels run once per ub_step)
-TRAFFIC_BYTES_PER_LAUNCH = 463.3e6   # dram read+write bytes of the two ub::k_stream launches of one round, profiles/r01f_stream.md
+TRAFFIC_BYTES_PER_LAUNCH = 463.3e6   # dram read+write bytes of the two ub::k_stream launches of one round, profiles/r01g_stream.md
 ALG_BYTES_PER_REQUEST_STEP = 40      # read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
 METRIC = "request-steps scheduled/sec"
 UNIT = "request-steps/s"
