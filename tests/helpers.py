@@ -1,4 +1,7 @@
 """Shared test helpers: small seeded memory-pressured traces (inputs only, no scheduler arithmetic)."""
+import json
+import os
+
 import numpy as np
 
 from paper_2606_18431_b200 import workloads as W
@@ -21,3 +24,19 @@ def pressure_workload(seed, n=60, kv_blocks=48, policy=W.POLICY_BOOST, gamma=0.3
                swap_pool_blocks=kv_blocks, max_batch=16, chunk_tokens=64, token_budget=96)
     sim.update(sim_kw)
     return W.custom(a, P, D, sim, rep, name=f"pressure{seed}")
+
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def hand_cases():
+    """The hand-worked schedules of tests/golden/hand_traces.{md,json} (inputs and expected numbers, all typed by hand)."""
+    with open(os.path.join(GOLD, "hand_traces.json")) as f:
+        return json.load(f)["cases"]
+
+
+def hand_workload(case):
+    sim = dict(block_tokens=16, c0_us=1000, c_prefill_tok_us=10, c_decode_seq_us=100, queue_cap=8)
+    sim.update(case["sim"])
+    rep = W.make_replicas(1, hysteresis_us=0, **case["replica"])
+    return W.custom(case["arrival_us"], case["prompt"], case["decode"], sim, rep, name=case["name"])

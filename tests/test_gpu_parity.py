@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 from paper_2606_18431_b200 import workloads as W
-from tests.helpers import pressure_workload
+from tests.helpers import hand_cases, hand_workload, pressure_workload
 
 pytestmark = pytest.mark.gpu
 
@@ -68,6 +68,39 @@ def test_boost_table_bit_exact(gpu, oracle_mod, gamma, quant):
     wl = pressure_workload(1, n=40, gamma=gamma, quant=quant)
     g, o = _pair(gpu, oracle_mod, wl)
     assert np.array_equal(g.boost_lut(0), o.boost_lut(0))
+
+
+# ------------------------------------------------------------------------------------------ hand-worked schedules
+
+@pytest.mark.parametrize("case", hand_cases(), ids=[c["name"] for c in hand_cases()])
+def test_hand_worked_schedules_on_the_device(gpu, oracle_mod, case):
+    """tests/golden/hand_traces.md (A-J): the CUDA path against the numbers derived by hand from Algorithm 1
+     -- the PHASE signal, the AUTO swap rule, swap-time rounding, the one-token prefill tail among
+    them -- iteration by iteration, and against the oracle."""
+    wl = hand_workload(case)
+    exp = case["expect"]
+    g, o = _pair(gpu, oracle_mod, wl)
+    t_prev, costs = 0, []
+    for it in range(len(exp["step_costs_us"])):
+        g.step(1)
+        info, _ = o.step_replica(0)
+        t = g.debug_state(0)["clock_us"]
+        assert t == info["t_end_us"], f"iteration {it}"
+        costs.append(t - info["t_start_us"])
+        assert g.digest()[0] == o.digest()[0], f"iteration {it}"
+    assert costs == exp["step_costs_us"]
+    assert g.step(1, want_live=True) == 0
+    n = len(case["prompt"])
+    tf, tl, ne, neu = g.per_request()
+    assert tf[0, :n].tolist() == exp["t_first_us"] and tl[0, :n].tolist() == exp["t_last_us"]
+    assert ne[0, :n].tolist() == exp["n_evict"]
+    if "n_evict_unforced" in exp:
+        assert neu[0, :n].tolist() == exp["n_evict_unforced"]
+    st = g.stats()[0]
+    for k in ("iterations", "request_steps", "t_end_us", "tokens_lost", "prefill_tokens", "decode_seqs",
+              "evict_recompute", "evict_swap") + (("swapins",) if "swapins" in exp else ()):
+        assert st[k] == exp[k], k
+    _assert_same(g, o, case["name"])
 
 
 # ------------------------------------------------------------------------------------------ config 1 in full

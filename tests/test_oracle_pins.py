@@ -16,9 +16,7 @@ import pytest
 
 from oracle import oracle as O
 from paper_2606_18431_b200 import workloads as W
-from tests.helpers import pressure_workload
-
-GOLD = os.path.join(os.path.dirname(__file__), "golden")
+from tests.helpers import GOLD, hand_cases, hand_workload, pressure_workload
 
 
 def run_wl(wl, **kw):
@@ -29,15 +27,8 @@ def run_wl(wl, **kw):
 
 # ------------------------------------------------------------------ hand-worked schedules
 
-with open(os.path.join(GOLD, "hand_traces.json")) as f:
-    HAND = json.load(f)["cases"]
-
-
-def _hand_workload(case):
-    sim = dict(block_tokens=16, c0_us=1000, c_prefill_tok_us=10, c_decode_seq_us=100, queue_cap=8)
-    sim.update(case["sim"])
-    rep = W.make_replicas(1, hysteresis_us=0, **case["replica"])
-    return W.custom(case["arrival_us"], case["prompt"], case["decode"], sim, rep, name=case["name"])
+HAND = hand_cases()
+_hand_workload = hand_workload
 
 
 @pytest.mark.parametrize("case", HAND, ids=[c["name"] for c in HAND])
@@ -53,14 +44,16 @@ def test_hand_worked_schedule(case):
             break
         costs.append(info["cost_us"])
     assert costs == exp["step_costs_us"]
-    tf, tl, ne, _ = sim.per_request()
+    tf, tl, ne, neu = sim.per_request()
     n = len(case["prompt"])
     assert tf[0, :n].tolist() == exp["t_first_us"]
     assert tl[0, :n].tolist() == exp["t_last_us"]
     assert ne[0, :n].tolist() == exp["n_evict"]
+    if "n_evict_unforced" in exp:
+        assert neu[0, :n].tolist() == exp["n_evict_unforced"]
     st = sim.stats()[0]
     for k in ("iterations", "request_steps", "t_end_us", "tokens_lost", "prefill_tokens", "decode_seqs",
-              "evict_recompute", "evict_swap"):
+              "evict_recompute", "evict_swap") + (("swapins",) if "swapins" in exp else ()):
         assert st[k] == exp[k], k
     assert st["done"] == 1 and st["n_completed"] == n
 
