@@ -75,7 +75,10 @@ __device__ __forceinline__ void score(const Rec0& q0, const Rec1& q1, uint32_t k
 }
 
 // ADA: the gamma-Ada instance (per-level boost tables, latency window); the static instance carries none of it.
-template <bool ADA>
+// MULTI: several iterations per launch (the resident-state mode: the window is re-read from L2 between them); the
+// one-iteration instance carries none of that either -- the instruction cache (32 KB per SM) is what this kernel
+// competes for, so every instance holds only the code it runs.
+template <bool ADA, bool MULTI>
 __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   __shared__ WarpBuf wbuf[kSWarps];
   const SimDev& s = A.s;
@@ -102,18 +105,22 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   // striding (3/4 of an even share); the rest are handed out dynamically: each is the next value of a global ticket
   // counter (count[4] / count[6] alternately, each zeroed by the launch before), requested one replica ahead so that the atomic's latency is never waited for.
 #define UB_GW (A.rbeg + blockIdx.x * kSWarps + (threadIdx.x >> 5))
-  uint32_t r = UB_GW, rn = UB_GW + nwarps;
-  uint32_t taken = 2, ticket = 0;
-  uint32_t parity = 0;
-  prefetch_replica(r, 0);
+  // r: the replica being advanced (its header and first chunks sit in stage `parity`), rn: the one being fetched; the
+  // first round of the loop only fetches (one prefetch site: code size)
+  constexpr uint32_t kNone = 0xFFFFFFFFu;
+  uint32_t r = kNone, rn = UB_GW;
+  uint32_t taken = 1, ticket = 0;
+  uint32_t parity = 1;
   // (the ticket counter of the NEXT launch is zeroed here: launches of one part alternate between the two)
   if (blockIdx.x == 0 && threadIdx.x == 0) A.count[4 + 2 * (A.tick ^ 1u)] = 0u;
-  for (; r < A.rend; r = rn, rn = (taken < A.nstat ? UB_GW + taken * nwarps : __shfl_sync(kFull, ticket, 0) + A.dynbase), taken++,
-                  parity ^= 1u) {
+  for (;; r = rn, rn = (taken < A.nstat ? UB_GW + taken * nwarps : __shfl_sync(kFull, ticket, 0) + A.dynbase), taken++,
+          parity ^= 1u) {
     cp_wait<0>();
     __syncwarp();
     prefetch_replica(rn, parity ^ 1u);
     if (taken >= A.nstat && lane == 0) ticket = atomicAdd(A.count + 4 + 2 * A.tick, 1u);
+    if (r == kNone) continue;
+    if (r >= A.rend) break;
     const unsigned long long* sh = reinterpret_cast<const unsigned long long*>(X.hdr[parity]);
     // (addresses and per-replica scalars that are needed rarely are re-derived where they are used instead of
     // living in registers across the chunk loop)
@@ -131,7 +138,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       }
     }
     uint32_t nd = (uint32_t)sh[18];                                   // entries of the dirty list
-    const uint32_t iters = A.iters;
+    const uint32_t iters = MULTI ? A.iters : 1u;
     const RepPar par = reinterpret_cast<const Hdr*>(X.hdr[parity])->par;
     Rec0* gE0 = s.E0 + (size_t)r * Q;
     Rec1* gE1 = s.E1 + (size_t)r * Q;
@@ -184,7 +191,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         }
         cp_commit();
       };
-      if (it > 0) {                                                   // (the first iteration found them prefetched)
+      if (MULTI && it > 0) {                                          // (the first iteration found them prefetched)
         cp16(&X.spec[parity][0][lane], reinterpret_cast<const uint4*>(gE0) + lane);
         cp16(&X.spec[parity][0][32 + lane], reinterpret_cast<const uint4*>(gE1) + lane);
         cp16(&X.spec[parity][1][lane], reinterpret_cast<const uint4*>(gE0) + 32 + lane);
@@ -199,17 +206,22 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       // ---------------- a2 (first half): the requests that may change place -- dirty ones and arrivals -- are taken
       // out of the stream, scored, ranked among themselves by (class, key, id) and parked in shared memory
       uint32_t spos = 0xFFFFFFFFu;                                    // window position a dirty request is taken from
+      uint32_t dlo = 0, dspan = 0;                                    // chunks [dlo, dlo + dspan) hold the positions they are taken from
       if (m) {
         int4 v0 = make_int4(0, 0, 0, 0), v1 = make_int4(0, 0, 0, 0);
         if ((uint32_t)lane < nd) {
-          spos = it == 0 ? (uint32_t)reinterpret_cast<const Hdr*>(X.hdr[parity])->dl[lane]
-                         : (uint32_t)__ldcg(s.hdr[r].dl + lane);
+          spos = (!MULTI || it == 0) ? (uint32_t)reinterpret_cast<const Hdr*>(X.hdr[parity])->dl[lane]
+                                     : (uint32_t)__ldcg(s.hdr[r].dl + lane);
           v0 = __ldcg(reinterpret_cast<const int4*>(gE0 + spos));
           v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + spos));
         } else if ((uint32_t)lane < m) {
           const uint32_t i = next + ((uint32_t)lane - nd);
           v0 = __ldg(reinterpret_cast<const int4*>(UB_TR + i));
           v1 = make_int4((int)i, 0, 0, 0);
+        }
+        if (nd) {
+          dlo = __reduce_min_sync(kFull, spos >> 5);                  // (lanes without a dirty request hold 0xFFFFFFFF)
+          dspan = __reduce_max_sync(kFull, (uint32_t)lane < nd ? spos >> 5 : 0u) - dlo + 1u;
         }
         if (cnt) {
           next += cnt;
@@ -227,6 +239,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         score(q0, q1, k, lutv, UB_DELTA, guard, sk, sb);
         uint32_t rank = 0;
         if (m > 1u) {
+#pragma unroll 1
           for (uint32_t j = 0; j < m; j++) {
             const uint64_t kj = __shfl_sync(kFull, sk, (int)j);
             const uint32_t ij = __shfl_sync(kFull, q1.id, (int)j);
@@ -239,7 +252,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           X.skb[rank] = make_uint4((uint32_t)sk, (uint32_t)(sk >> 32), sb, 0u);
         }
       }
-      if (it > 0) { if (nch > 2u) cp_wait<kRing>(); else cp_wait<0>(); }   // the re-read chunks 0, 1
+      // the re-read chunks 0, 1; with parked requests the stores of chunk 1 may reach into chunk 2: it must have landed
+      if (nch > 2u) { if (m) cp_wait<kRing - 1>(); else if (MULTI && it > 0) cp_wait<kRing>(); } else if (MULTI && it > 0) cp_wait<0>();
       __syncwarp();
 
       // ---------------- the pass.  Walk state (M7), warp-uniform: mode 0 = everybody walks, 1 = residents only (a
@@ -249,6 +263,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       // per-lane sums: de = decode sequences | tokens emitted << 16; ps = prefill tokens | same-gap emissions << 16
       // (each field < 2^16: M, Q <= 2048, T <= 65535); swap-ins (rare) are summed in shared memory
       uint32_t de = 0, ps = 0, kres = 0, evl = 0, evu = 0;
+      uint32_t rhi = 0;                                               // 1 + the last new position this lane gave to a resident
       if (lane == 0) X.skb[0].w = 0u, X.skb[1].w = 0u;                // (the spare words of the parking area)
       uint32_t outpos = 0, nev = 0, ndnew = 0, n_done = 0;
       uint32_t dptr = 0;                                              // next parked request to merge
@@ -379,6 +394,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const bool keep = (keepm >> lane) & 1u;
         const uint32_t np = outpos + __popc(keepm & ltmask);
         const bool moved = np != stpos;
+        if (keep && res2 && np >= rhi) rhi = np + 1u;
         if (keep && moved) __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&w0));
         if (keep && (moved || adm || nf != of))
           __stcg(reinterpret_cast<int4*>(gE1 + np), make_int4((int)w1.id, (int)d2, (int)cached2, (int)nf));
@@ -392,69 +408,55 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         n_done += __popc(gonem);
       };
 
-      for (uint32_t c = 0; c <= nch; c++) {
-        if (c == nch && dptr >= m) break;                             // (chunk nch is empty: the parked tail)
-        // the chunk must have landed; when parked requests are merged in, the writes of this chunk may reach into
-        // the next one, which must then have landed too before anything is stored
-        if (c >= 2u) { if (m) cp_wait<kRing - 2>(); else cp_wait<kRing - 1>(); __syncwarp(); }
-        else if (c == 1u && m && nch > 2u) { cp_wait<kRing - 1>(); __syncwarp(); }
-        const uint4* st = c < 2u ? X.spec[parity][c] : X.ring[(c - 2u) % kRing];
-        const uint4 c0 = st[lane], c1 = st[32 + lane];
-        if (c >= 2u) { __syncwarp(); issue_chunk(c + kRing); }        // the stage is free again
-        const Rec0 r0 = *reinterpret_cast<const Rec0*>(&c0);
-        const Rec1 r1 = *reinterpret_cast<const Rec1*>(&c1);
+      // The pass over the chunks.  Three phases share the walk state: (A) a run of chunks of MemGuard-locked residents
+      // in steady decode, (T) the tail of steadily waiting requests behind the walk, (G) everything else, one chunk
+      // at a time.  A lane reads back from the stages exactly the 32 bytes it copied itself, so the asynchronous
+      // copies need no warp barrier; cp.async.wait_group alone orders them.
+      auto stage_of = [&](const uint32_t c) -> const uint4* { return c < 2u ? X.spec[parity][c] : X.ring[(c - 2u) % kRing]; };
+      // chunk c (>= 2) must have landed; when parked requests were merged in, the writes of a chunk may reach into
+      // the next one, which must then have landed too before anything is stored (two predicated waits, no branch)
+      auto wait_chunk = [&](const uint32_t c) {
+        if (c >= 2u)
+          asm volatile("{ .reg .pred p; setp.ne.u32 p, %0, 0; @p cp.async.wait_group %1; @!p cp.async.wait_group %2; }"
+                       :: "r"(m), "n"(kRing - 2), "n"(kRing - 1) : "memory");
+      };
+      // requests of chunk c still in the stream (the dirty ones were taken out)
+      auto valid_of = [&](const uint32_t c) -> uint32_t {
         const uint32_t left = c < nch ? n_old - c * 32u : 0u;
-        uint32_t cv = left >= 32u ? kFull : ((1u << left) - 1u);      // requests of this chunk still in the stream
-        if (nd) cv &= ~__reduce_or_sync(kFull, ((uint32_t)lane < nd && (spos >> 5) == c) ? (1u << (spos & 31u)) : 0u);
-        // the next parked request, if any: fast paths apply only to chunks that sort in front of it
-        const bool pend = dptr < m;
-        uint32_t pk_lo = 0, pk_hi = 0, pk_id = 0;
-        if (pend) { const uint4 dk = X.skb[dptr]; pk_lo = dk.x; pk_hi = dk.y; pk_id = X.sr1[dptr].x; }
-        uint64_t key = 0; uint32_t bin = 0;
-        bool scored = false;
-        if (mode != 0u && cv != 0u) {
-          // ---- behind the walk: a chunk of waiting requests (not resident, nothing to finalise) only moves up
-          const bool steady = (r1.flags & ~F_SWAPPED) == F_KLASS1;
-          if (__all_sync(kFull, steady || !((cv >> lane) & 1u))) {
-            bool before = true;
-            if (pend) {
-              score(r0, r1, k, lutv, UB_DELTA, guard, key, bin);
-              scored = true;
-              const int last = 31 - __clz((int)cv);
-              const uint64_t lk = __shfl_sync(kFull, key, last);
-              const uint32_t li = __shfl_sync(kFull, r1.id, last);
-              before = key_less(lk, li, (uint64_t)pk_lo | ((uint64_t)pk_hi << 32), pk_id);
-            }
-            if (before) {
-              const uint32_t np = outpos + __popc(cv & ltmask);
-              if (np != c * 32u + (uint32_t)lane && ((cv >> lane) & 1u)) {
-                __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
-                __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
-              }
-              outpos += __popc(cv);
-              continue;
-            }
-          }
-        }
-        if (mode == 0u && guard && cv != 0u && (!pend || (pk_hi >> 31))) {
-          // ---- a chunk of MemGuard-locked residents in steady decode (each wants one token, emits it, neither
-          // completes nor crosses its Eq. 8 threshold) that fits as a whole: class 0 in stored order (so in front of
-          // a parked request of class 1), nothing is re-keyed, every record advances by one token (M2, M7, M10)
-          const bool valid = (cv >> lane) & 1u;
-          const uint32_t fl = r1.flags;
-          const uint32_t sig1 = r0.P + r1.d + 1u;                      // signal after this token
-          const bool okl = (fl & (F_LOCK_MASK_LOW)) == (F_RESIDENT | F_ADMITNOW | F_EMITPREV) && r1.cached + 2u == sig1 &&
-                           r1.d + 1u != r0.D && sig1 != (k << (fl >> F_LOCK_SHIFT));
-          // ... optionally followed, when nothing is parked, by steadily waiting requests (not resident, nothing to
-          // finalise) whose first one is turned away -- on KV ("newblocked": the walk goes on over residents only,
-          // of which this chunk has none left) or because the batch / token budget is used up (the walk stops)
-          const bool okw = !okl && (fl & ~F_SWAPPED) == F_KLASS1;
-          const uint32_t decm = __ballot_sync(kFull, valid && okl);
-          const uint32_t wm = pend ? 0u : __ballot_sync(kFull, valid && okw);
-          if ((decm | wm) == cv && (wm == 0u || decm < (wm & (0u - wm)))) {    // (decoders first)
-            const uint32_t nv = __popc(decm);
-            const uint32_t totf = __reduce_add_sync(kFull, (valid && okl) ? (r1.cached + 1u + blk_m1) >> blk_sh : 0u);
-            if (crank + nv <= M && carryW + nv <= Tb && carryC + totf <= B) {
+        uint32_t cv = left >= 32u ? kFull : ((1u << left) - 1u);
+        if (c - dlo < dspan) cv &= ~__reduce_or_sync(kFull, ((uint32_t)lane < nd && (spos >> 5) == c) ? (1u << (spos & 31u)) : 0u);
+        return cv;
+      };
+      uint32_t c = 0;
+      for (;;) {
+        // ---------------- (A) chunks of MemGuard-locked residents in steady decode (each wants one token, emits it,
+        // neither completes nor crosses its Eq. 8 threshold) that fit as a whole: class 0 in stored order (so in front
+        // of a parked request of class 1), nothing is re-keyed, every record advances by one token (M2, M7, M10)
+        if (mode == 0u && guard && c < nch) {
+          const bool pend = dptr < m;
+          if (!pend || (X.skb[dptr].y >> 31)) {
+            do {
+              wait_chunk(c);
+              const uint4* st = stage_of(c);
+              const uint4 c0 = st[lane], c1 = st[32 + lane];
+              const Rec0 r0 = *reinterpret_cast<const Rec0*>(&c0);
+              const Rec1 r1 = *reinterpret_cast<const Rec1*>(&c1);
+              const uint32_t cv = valid_of(c);
+              const bool valid = (cv >> lane) & 1u;
+              const uint32_t fl = r1.flags;
+              const uint32_t sig1 = r0.P + r1.d + 1u;                  // signal after this token
+              const bool okl = (fl & (F_LOCK_MASK_LOW)) == (F_RESIDENT | F_ADMITNOW | F_EMITPREV) && r1.cached + 2u == sig1 &&
+                               r1.d + 1u != r0.D && sig1 != (k << (fl >> F_LOCK_SHIFT));
+              // ... optionally followed, when nothing is parked, by steadily waiting requests (not resident, nothing
+              // to finalise) whose first one is turned away -- on KV ("newblocked": the walk goes on over residents
+              // only, of which this chunk has none left) or because the batch / token budget is used up (walk stops)
+              const bool okw = !okl && (fl & ~F_SWAPPED) == F_KLASS1;
+              const uint32_t decm = __ballot_sync(kFull, valid && okl);
+              const uint32_t wm = pend ? 0u : __ballot_sync(kFull, valid && okw);
+              if ((decm | wm) != cv || cv == 0u || (wm != 0u && decm >= (wm & (0u - wm)))) break;   // (decoders first)
+              const uint32_t nv = __popc(decm);
+              const uint32_t totf = __reduce_add_sync(kFull, (valid && okl) ? (r1.cached + 1u + blk_m1) >> blk_sh : 0u);
+              if (crank + nv > M || carryW + nv > Tb || carryC + totf > B) break;
               uint32_t nmode = 0;
               if (wm) {
                 const uint32_t tokb = carryW + nv, cbw = crank + nv;
@@ -466,59 +468,131 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
                   const uint32_t footw = __shfl_sync(kFull, (r1.cached + wnt + blk_m1) >> blk_sh, __ffs(wm) - 1);
                   nmode = (carryC + totf + footw > B) ? 1u : 3u;       // 3: it is admitted -> general path
                 }
+                if (nmode == 3u) break;
               }
-              if (nmode != 3u) {
-                const uint32_t np = outpos + __popc(cv & ltmask);
-                const bool moved = np != c * 32u + (uint32_t)lane;
-                if (valid && moved) __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
-                if (valid && okl) {
-                  __stcg(reinterpret_cast<int4*>(gE1 + np),
-                         make_int4((int)r1.id, (int)(r1.d + 1u), (int)(r1.cached + 1u), (int)fl));
-                  const uint64_t h = (uint64_t)(((r1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu)) * 3ull;
-                  evl += (uint32_t)h; evu += (uint32_t)(h >> 32);
-                  de += 0x10001u; ps += 0x10000u;
-                } else if (valid && moved) {
-                  __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
-                }
-                carryW += nv; carryC += totf; carryN = crank + nv;     // (carryN: the turned-away request's rank)
-                crank += __popc(cv); outpos += __popc(cv);
-                mode = nmode;
-                continue;
+              const uint32_t np = outpos + __popc(cv & ltmask);
+              const bool moved = np != c * 32u + (uint32_t)lane;
+              if (valid && moved) __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
+              if (valid && okl) {
+                __stcg(reinterpret_cast<int4*>(gE1 + np),
+                       make_int4((int)r1.id, (int)(r1.d + 1u), (int)(r1.cached + 1u), (int)fl));
+                const uint64_t h = (uint64_t)(((r1.id + 1u) * 0x9E3779B1u) ^ ((uint32_t)EV_ADMIT * 0x85EBCA6Bu)) * 3ull;
+                evl += (uint32_t)h; evu += (uint32_t)(h >> 32);
+                de += 0x10001u; ps += 0x10000u;
+                rhi = np + 1u > rhi ? np + 1u : rhi;
+              } else if (valid && moved) {
+                __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
               }
+              carryW += nv; carryC += totf; carryN = crank + nv;       // (carryN: the turned-away request's rank)
+              crank += __popc(cv); outpos += __popc(cv);
+              mode = nmode;
+              if (c >= 2u) issue_chunk(c + kRing);                     // the stage is free again
+              c++;
+            } while (mode == 0u && c < nch);
+          }
+        }
+        // ---------------- (T) behind the walk, nothing parked left: chunks of waiting requests (not resident, nothing
+        // to finalise) only move up when requests in front of them completed
+        if (mode != 0u && dptr >= m && c >= dlo + dspan) {
+          while (c < nch) {
+            wait_chunk(c);
+            const uint4* st = stage_of(c);
+            const uint32_t fl = reinterpret_cast<const uint32_t*>(st + 32 + lane)[3];
+            const uint32_t left = n_old - c * 32u;
+            const bool valid = (uint32_t)lane < left;
+            if (!__all_sync(kFull, (fl & ~F_SWAPPED) == F_KLASS1 || !valid)) break;
+            const uint32_t np = outpos + (uint32_t)lane;
+            if (outpos != c * 32u && valid) {
+              const uint4 c0 = st[lane], c1 = st[32 + lane];
+              __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
+              __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
+            }
+            outpos += left < 32u ? left : 32u;
+            if (c >= 2u) issue_chunk(c + kRing);
+            c++;
+          }
+        }
+        if (c > nch || (c == nch && dptr >= m)) break;                // (chunk nch is empty: the parked tail)
+
+        // ---------------- (G) one chunk on the general path
+        wait_chunk(c);
+        const uint4* st = stage_of(c);
+        const uint4 c0 = st[lane], c1 = st[32 + lane];
+        if (c >= 2u) issue_chunk(c + kRing);                          // the stage is free again
+        const Rec0 r0 = *reinterpret_cast<const Rec0*>(&c0);
+        const Rec1 r1 = *reinterpret_cast<const Rec1*>(&c1);
+        const uint32_t cv = valid_of(c);
+        uint64_t key; uint32_t bin;
+        score(r0, r1, k, lutv, UB_DELTA, guard, key, bin);
+        if (mode != 0u && cv != 0u) {
+          // ---- behind the walk: a chunk of waiting requests (not resident, nothing to finalise) that sorts in front
+          // of the next parked request, if any, only moves up
+          const bool steady = (r1.flags & ~F_SWAPPED) == F_KLASS1;
+          if (__all_sync(kFull, steady || !((cv >> lane) & 1u))) {
+            bool before = true;
+            if (dptr < m) {
+              const uint4 dk = X.skb[dptr];
+              const uint32_t pk_id = X.sr1[dptr].x;
+              const int last = 31 - __clz((int)cv);
+              const uint64_t lk = __shfl_sync(kFull, key, last);
+              const uint32_t li = __shfl_sync(kFull, r1.id, last);
+              before = key_less(lk, li, (uint64_t)dk.x | ((uint64_t)dk.y << 32), pk_id);
+            }
+            if (before) {
+              const uint32_t np = outpos + __popc(cv & ltmask);
+              if (np != c * 32u + (uint32_t)lane && ((cv >> lane) & 1u)) {
+                __stcg(reinterpret_cast<int4*>(gE0 + np), *reinterpret_cast<const int4*>(&c0));
+                __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
+              }
+              outpos += __popc(cv);
+              c++;
+              continue;
             }
           }
         }
-        if (!scored) score(r0, r1, k, lutv, UB_DELTA, guard, key, bin);
-        uint32_t lo = 0;
+        // the merged order of this chunk: alternately a run of its clean requests (up to the first one that sorts
+        // behind the next parked request) and the parked requests that sort in front of that one
+        uint32_t lo = 0, fl = 32;
+        bool turn = false;                                            // false: clean run, true: parked run
+#pragma unroll 1
         for (;;) {
-          uint32_t fl = 32;
-          if (dptr < m) {                                             // clean requests that sort behind the next parked one
-            const uint4 dk = X.skb[dptr];
-            const uint32_t di = X.sr1[dptr].x;
-            const uint32_t after = __ballot_sync(kFull, ((cv >> lane) & 1u) && (uint32_t)lane >= lo &&
-                                                 key_less((uint64_t)dk.x | ((uint64_t)dk.y << 32), di, key, r1.id));
-            if (after) fl = (uint32_t)__ffs(after) - 1u;
-          }
-          const uint32_t seg = cv & (fl < 32u ? ((1u << fl) - 1u) : kFull) & (lo < 32u ? (kFull << lo) : 0u);
-          if (seg) process(r0, r1, key, bin, seg, c * 32u + (uint32_t)lane);
-          lo = fl;
-          if ((fl == 32u && c < nch) || dptr >= m) break;
-          uint32_t j = m - dptr;                                      // parked requests in front of clean lane fl
-          if (fl < 32u) {
-            const uint64_t ck = __shfl_sync(kFull, key, (int)fl);
-            const uint32_t ci = __shfl_sync(kFull, r1.id, (int)fl);
-            const uint4 kb = X.skb[lane];
-            j = __popc(__ballot_sync(kFull, (uint32_t)lane >= dptr && (uint32_t)lane < m &&
-                                     key_less((uint64_t)kb.x | ((uint64_t)kb.y << 32), X.sr1[lane].x, ck, ci)));
-          }
-          {
+          Rec0 w0 = r0; Rec1 w1 = r1; uint64_t wk = key; uint32_t wb = bin, wmask, wst = c * 32u + (uint32_t)lane;
+          uint32_t j = 0;
+          if (!turn) {
+            fl = 32;
+            if (dptr < m) {                                           // clean requests that sort behind the next parked one
+              const uint4 dk = X.skb[dptr];
+              const uint32_t di = X.sr1[dptr].x;
+              const uint32_t after = __ballot_sync(kFull, ((cv >> lane) & 1u) && (uint32_t)lane >= lo &&
+                                                   key_less((uint64_t)dk.x | ((uint64_t)dk.y << 32), di, key, r1.id));
+              if (after) fl = (uint32_t)__ffs(after) - 1u;
+            }
+            wmask = cv & (fl < 32u ? ((1u << fl) - 1u) : kFull) & (lo < 32u ? (kFull << lo) : 0u);
+          } else {
+            j = m - dptr;                                             // parked requests in front of clean lane fl
+            if (fl < 32u) {
+              const uint64_t ck = __shfl_sync(kFull, key, (int)fl);
+              const uint32_t ci = __shfl_sync(kFull, r1.id, (int)fl);
+              const uint4 kb = X.skb[lane];
+              j = __popc(__ballot_sync(kFull, (uint32_t)lane >= dptr && (uint32_t)lane < m &&
+                                       key_less((uint64_t)kb.x | ((uint64_t)kb.y << 32), X.sr1[lane].x, ck, ci)));
+            }
             const uint32_t src = dptr + (uint32_t)lane < 32u ? dptr + (uint32_t)lane : 31u;
             const uint4 a0 = X.sr0[src], a1 = X.sr1[src], ak = X.skb[src];
-            process(*reinterpret_cast<const Rec0*>(&a0), *reinterpret_cast<const Rec1*>(&a1),
-                    (uint64_t)ak.x | ((uint64_t)ak.y << 32), ak.z, j < 32u ? ((1u << j) - 1u) : kFull, 0xFFFFFFFFu);
+            w0 = *reinterpret_cast<const Rec0*>(&a0); w1 = *reinterpret_cast<const Rec1*>(&a1);
+            wk = (uint64_t)ak.x | ((uint64_t)ak.y << 32); wb = ak.z;
+            wmask = j < 32u ? ((1u << j) - 1u) : kFull; wst = 0xFFFFFFFFu;
           }
-          dptr += j;
+          if (wmask) process(w0, w1, wk, wb, wmask, wst);
+          if (!turn) {
+            lo = fl;
+            if ((fl == 32u && c < nch) || dptr >= m) break;
+          } else {
+            dptr += j;
+          }
+          turn = !turn;
         }
+        c++;
       }
       __syncwarp();
 
@@ -546,7 +620,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         // of blocks exceeds B - C; lowest priority first, the swap pool being a sequential resource.
         const uint32_t thr = B - C;
         uint32_t behind = 0;                                          // blocks of stalled residents behind this chunk
-        for (int c = (int)((n_new - 1u) >> 5); c >= 0; c--) {
+        // (behind the last resident there is nothing to look at)
+        for (int c = (int)((__reduce_max_sync(kFull, rhi) - 1u) >> 5); c >= 0; c--) {
           const uint32_t pos = (uint32_t)c * 32u + (uint32_t)lane;
           int4 v1 = make_int4(0, 0, 0, 0);
           if (pos < n_new) v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + pos));
@@ -609,6 +684,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         int64_t* g_tfirst = s.t_first + (size_t)r * s.N;
         int64_t* g_tlast = s.t_last + (size_t)r * s.N;
         uint32_t cseq = ADA ? (uint32_t)reinterpret_cast<const unsigned long long*>(X.hdr[parity])[15] : 0u;   // completions so far
+#pragma unroll 1
         for (uint32_t e0 = 0; e0 < nev; e0 += 32u) {
           const uint32_t e = e0 + (uint32_t)lane;
           uint32_t cm = 0;
@@ -683,7 +759,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         it++;
         break;
       }
-      __syncwarp();                                                   // window stores before the next iteration's loads
+      if (MULTI) __syncwarp();                                        // window stores before the next iteration's loads
     }
 
     // ---------------- not handled here: queue the replica for the team kernels of this round
@@ -700,12 +776,12 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 }
 
 // persistent grid: every warp takes replicas until none is left
-template <bool ADA> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
+template <bool ADA, bool MULTI> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
   StepArgs A = A0;
   static int ctas_per_sm = 0;
   if (!ctas_per_sm) {
-    cudaFuncSetAttribute(k_stream<ADA>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream<ADA>, 32 * kSWarps, 0) != cudaSuccess ||
+    cudaFuncSetAttribute(k_stream<ADA, MULTI>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream<ADA, MULTI>, 32 * kSWarps, 0) != cudaSuccess ||
         ctas_per_sm < 1)
       ctas_per_sm = 4;
   }
@@ -719,10 +795,12 @@ template <bool ADA> static void launch_stream_t(const StepArgs& A0, cudaStream_t
   const uint32_t nwarps = grid * kSWarps, share = ((A.rend - A.rbeg) / nwarps) * 3u / 4u;
   A.nstat = share > 2u ? share : 2u;
   A.dynbase = A.rbeg + A.nstat * nwarps;
-  k_stream<ADA><<<grid, 32 * kSWarps, 0, st>>>(A);
+  k_stream<ADA, MULTI><<<grid, 32 * kSWarps, 0, st>>>(A);
 }
 void launch_stream(const StepArgs& A, cudaStream_t st) {
-  if (A.s.ada_ring) launch_stream_t<true>(A, st); else launch_stream_t<false>(A, st);
+  if (A.s.ada_ring) launch_stream_t<true, false>(A, st);          // (gamma-Ada: one iteration per launch, ub_api.cu)
+  else if (A.iters > 1u) launch_stream_t<false, true>(A, st);
+  else launch_stream_t<false, false>(A, st);
 }
 
 }  // namespace ub
