@@ -61,7 +61,7 @@ typedef struct {
   uint32_t abi_version;           /* UB_ABI_VERSION */
   uint32_t n_replicas;            /* R >= 1 */
   uint32_t n_traces;              /* distinct traces; replicas may share one */
-  uint32_t max_requests;          /* N: row length of the trace arrays */
+  uint32_t max_requests;          /* N: row length of the trace arrays, < 2^29 */
   uint32_t queue_cap;             /* Q: max simultaneously active requests per replica, 1..UB_MAX_QUEUE */
   uint32_t kv_blocks;             /* B: KV capacity in blocks */
   uint32_t block_tokens;          /* blk: tokens per block (16) */

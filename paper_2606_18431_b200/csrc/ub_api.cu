@@ -69,7 +69,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
   if (!c || !out) return UB_EINVAL;
   *out = nullptr;
   if (c->struct_size != sizeof(ub_config) || c->abi_version != UB_ABI_VERSION) return UB_EINVAL;
-  if (c->n_replicas < 1 || c->n_traces < 1 || c->max_requests < 1 || c->queue_cap < 1 ||
+  if (c->n_replicas < 1 || c->n_traces < 1 || c->max_requests < 1 || c->max_requests >= (1u << 29) || c->queue_cap < 1 ||
       c->queue_cap > UB_MAX_QUEUE || c->kv_blocks < 1 || c->block_tokens < 1 || c->max_batch < 1 ||
       c->chunk_tokens < 1 || c->chunk_tokens > 65535 || c->token_budget < 1 || c->token_budget > 65535 ||
       c->c0_us < 0 || c->c_prefill_tok_us < 0 || c->c_decode_seq_us < 0 || c->preempt_mode > 2 ||

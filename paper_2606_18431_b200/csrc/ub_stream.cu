@@ -31,6 +31,7 @@ namespace ub {
 constexpr int kSWarps = 4;                 // warps per CTA, each streams its own replicas
 constexpr int kRing = 4;                   // chunks in flight behind the two speculative ones
 constexpr uint32_t kFull = 0xffffffffu;
+constexpr uint32_t kEvSmem = 30;            // per-request events of one iteration kept in shared memory (spare words of skb[2..31])
 
 // inclusive warp scan, one SHFL + one predicated add per step (the shuffle's own "source lane in range" predicate)
 __device__ __forceinline__ uint32_t scan32(uint32_t v) {
@@ -118,7 +119,11 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     cp_wait<0>();
     __syncwarp();
     prefetch_replica(rn, parity ^ 1u);
-    if (taken >= A.nstat && lane == 0) ticket = atomicAdd(A.count + 4 + 2 * A.tick, 1u);
+    // (inline PTX: the compiler's own atomicAdd broadcasts the result with a shuffle at once, which waits ~600 cycles
+    // for the atomic's round trip -- 10 % of all warp time; here the ticket is first read one replica later)
+    if (taken >= A.nstat && lane == 0)
+      asm volatile("{ .reg .u64 a; .reg .u32 z; mov.u32 z, %%laneid; cvt.u64.u32 a, z; add.u64 a, a, %1; atom.global.add.u32 %0, [a], 1; }"
+                   : "=r"(ticket) : "l"(A.count + 4 + 2 * A.tick) : "memory");       // (lane 0: a = the counter)
     if (r == kNone) continue;
     if (r >= A.rend) break;
     const unsigned long long* sh = reinterpret_cast<const unsigned long long*>(X.hdr[parity]);
@@ -253,6 +258,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         }
       }
       // the re-read chunks 0, 1; with parked requests the stores of chunk 1 may reach into chunk 2: it must have landed
+      if (lane == 0) X.skb[0].w = 0u, X.skb[1].w = 0u;                // swap-in sums (spare words of the parking area; the
+                                                                      // barrier below orders the reset before their use)
       if (nch > 2u) { if (m) cp_wait<kRing - 1>(); else if (MULTI && it > 0) cp_wait<kRing>(); } else if (MULTI && it > 0) cp_wait<0>();
       __syncwarp();
 
@@ -264,7 +271,6 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       // (each field < 2^16: M, Q <= 2048, T <= 65535); swap-ins (rare) are summed in shared memory
       uint32_t de = 0, ps = 0, kres = 0, evl = 0, evu = 0;
       uint32_t rhi = 0;                                               // 1 + the last new position this lane gave to a resident
-      if (lane == 0) X.skb[0].w = 0u, X.skb[1].w = 0u;                // (the spare words of the parking area)
       uint32_t outpos = 0, nev = 0, ndnew = 0, n_done = 0;
       uint32_t dptr = 0;                                              // next parked request to merge
 
@@ -383,9 +389,12 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         if (__any_sync(kFull, defer || ends)) {
           if (ends) s.t_last[(size_t)r * s.N + w1.id] = (int64_t)sh[0];   // persist t_last when the streak ends
           const uint32_t em = __ballot_sync(kFull, defer);
-          if (defer)
-            s.evbuf[(size_t)r * s.evcap + nev + __popc(em & ltmask)] =
-                make_uint2(w1.id, (d_old == 0u ? 1u : 0u) | ((d_old != 0u && !ep_old) ? 2u : 0u) | (gone ? 4u : 0u));
+          if (defer) {                                                // the first kEvSmem of them wait in shared memory
+            const uint32_t slot = nev + __popc(em & ltmask);
+            const uint32_t kind = (d_old == 0u ? 1u : 0u) | ((d_old != 0u && !ep_old) ? 2u : 0u) | (gone ? 4u : 0u);
+            if (slot < kEvSmem) X.skb[2u + slot].w = (w1.id << 3) | kind;                 // (ids < 2^29: ub_create)
+            else s.evbuf[(size_t)r * s.evcap + slot] = make_uint2(w1.id, kind);
+          }
           nev += __popc(em);
         }
 
@@ -413,12 +422,11 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       // at a time.  A lane reads back from the stages exactly the 32 bytes it copied itself, so the asynchronous
       // copies need no warp barrier; cp.async.wait_group alone orders them.
       auto stage_of = [&](const uint32_t c) -> const uint4* { return c < 2u ? X.spec[parity][c] : X.ring[(c - 2u) % kRing]; };
-      // chunk c (>= 2) must have landed; when parked requests were merged in, the writes of a chunk may reach into
-      // the next one, which must then have landed too before anything is stored (two predicated waits, no branch)
-      auto wait_chunk = [&](const uint32_t c) {
-        if (c >= 2u)
-          asm volatile("{ .reg .pred p; setp.ne.u32 p, %0, 0; @p cp.async.wait_group %1; @!p cp.async.wait_group %2; }"
-                       :: "r"(m), "n"(kRing - 2), "n"(kRing - 1) : "memory");
+      // chunk c (>= 2) must have landed.  Stores go to positions at or below the ones read except after parked
+      // requests were merged in front: the writes of a chunk may then reach into the next one, which must have landed
+      // too before anything is stored (`ahead`: requests still parked, or the output position already in front)
+      auto wait_chunk = [&](const uint32_t c, const bool ahead) {
+        if (c >= 2u) { if (ahead) cp_wait<kRing - 2>(); else cp_wait<kRing - 1>(); }
       };
       // requests of chunk c still in the stream (the dirty ones were taken out)
       auto valid_of = [&](const uint32_t c) -> uint32_t {
@@ -436,7 +444,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           const bool pend = dptr < m;
           if (!pend || (X.skb[dptr].y >> 31)) {
             do {
-              wait_chunk(c);
+              wait_chunk(c, outpos > c * 32u);
               const uint4* st = stage_of(c);
               const uint4 c0 = st[lane], c1 = st[32 + lane];
               const Rec0 r0 = *reinterpret_cast<const Rec0*>(&c0);
@@ -495,7 +503,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         // to finalise) only move up when requests in front of them completed
         if (mode != 0u && dptr >= m && c >= dlo + dspan) {
           while (c < nch) {
-            wait_chunk(c);
+            wait_chunk(c, outpos > c * 32u);
             const uint4* st = stage_of(c);
             const uint32_t fl = reinterpret_cast<const uint32_t*>(st + 32 + lane)[3];
             const uint32_t left = n_old - c * 32u;
@@ -515,7 +523,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         if (c > nch || (c == nch && dptr >= m)) break;                // (chunk nch is empty: the parked tail)
 
         // ---------------- (G) one chunk on the general path
-        wait_chunk(c);
+        wait_chunk(c, dptr < m || outpos > c * 32u);
         const uint4* st = stage_of(c);
         const uint4 c0 = st[lane], c1 = st[32 + lane];
         if (c >= 2u) issue_chunk(c + kRing);                          // the stage is free again
@@ -674,8 +682,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           if (__ballot_sync(kFull, st) != allvm) break;               // a stalled resident that stays: so do all before it
         }
       }
-      const int64_t cost = s.c0 + s.c_pf * (int64_t)pf + s.c_dec * (int64_t)dec +
-                           (int64_t)(((uint64_t)(swin_blocks + swout_blocks) * s.swap_ns + 500u) / 1000u);
+      int64_t cost = s.c0 + s.c_pf * (int64_t)pf + s.c_dec * (int64_t)dec;
+      if (swin_blocks + swout_blocks) cost += (int64_t)(((uint64_t)(swin_blocks + swout_blocks) * s.swap_ns + 500u) / 1000u);
       const int64_t t_end = (int64_t)sh[0] + cost;
 
       // ---------------- the queued per-request events, now that t_end is known (M10, M11)
@@ -688,13 +696,13 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         for (uint32_t e0 = 0; e0 < nev; e0 += 32u) {
           const uint32_t e = e0 + (uint32_t)lane;
           uint32_t cm = 0;
-          if constexpr (ADA) {                                        // completions of this batch, in priority order
-            uint32_t kind = 0;
-            if (e < nev) kind = __ldcg(gev + e).y;
-            cm = __ballot_sync(kFull, (kind & 4u) != 0u);
-          }
+          uint2 ev = make_uint2(0u, 0u);
           if (e < nev) {
-            const uint2 ev = __ldcg(gev + e);
+            if (e < kEvSmem) { const uint32_t w = X.skb[2u + e].w; ev = make_uint2(w >> 3, w & 7u); }
+            else ev = __ldcg(gev + e);
+          }
+          if constexpr (ADA) cm = __ballot_sync(kFull, (ev.y & 4u) != 0u);   // completions of this batch, in priority order
+          if (e < nev) {
             const uint32_t id = ev.x;
             if (ev.y & 1u) {
               g_tfirst[id] = t_end;
