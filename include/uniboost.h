@@ -121,17 +121,24 @@ int  ub_load_trace(ub_sim*, const int64_t* arrival_us, const int32_t* prompt_tok
  * in fp64 (Eq. 2, rule M4) and uploads it.  Needs a loaded trace.  Synchronises. */
 int  ub_set_replicas(ub_sim*, const ub_replica* reps);
 
-/* Advance every replica by n_iters scheduler iterations (a0..a5 of DESIGN.md Sec. 2: ingest, score, order,
- * admit, victim-select, advance); finished replicas are no-ops.  Asynchronous on the stream unless
- * live_replicas (host, nullable) is given: then it synchronises and returns the number of unfinished replicas. */
+/* Advance every replica by n_iters scheduler iterations.  One iteration is one pass of Algorithm 1's loop body
+ * (PAPER.md:412-472): for all active r: SIGNAL -> QUANTIZE -> BOOST -> pi(r) = a_r - b_r -> UPDATEKEY;
+ * B <- {}, U <- KV usage; while |B| < M: r <- argmin of the queue tops, admit if U + KVNEED(r, c) <= B else
+ * SELECTVICTIM / SWAPOUT; EXECUTEONESTEP(B, c) under the stated cost model;
+ * UPDATESTATS -- steps a0..a5 of DESIGN.md Sec. 2, rules M6-M10.  Finished replicas are no-ops.
+ * Asynchronous on the stream unless live_replicas (host, nullable) is given: then it synchronises and returns the
+ * number of unfinished replicas. */
 int  ub_step(ub_sim*, uint32_t n_iters, uint64_t* live_replicas);
 
-/* Step until every replica is done or max_iters iterations were issued (then UB_ELIVELOCK).
- * iters_done (host, nullable) = iterations issued.  Synchronises. */
+/* Algorithm 1's outer loop ("while system is running") over the whole trace: ub_step until every replica
+ * has served its last request (trace exhausted and no request active, M6) or max_iters iterations were issued (then
+ * UB_ELIVELOCK).  iters_done (host, nullable) = iterations issued.  Synchronises. */
 int  ub_run(ub_sim*, uint64_t max_iters, uint64_t* iters_done);
 
-/* Device-resident reduction of the per-request histories to P50/P90/P99 TTFT / TTLT / TBT, means and
- * counters; out: host, [R].  Synchronises. */
+/* Device-resident reduction of the per-request histories to the tail metrics the paper reports (TTFT, TTLT = E2E
+ * and TBT at mean / P50 / P90 / P99: PAPER.md:245, 256-265): percentile p of m samples is the paper's
+ * t_p = inf{t : Fbar(t) <= (100 - p)/100} = the ceil(p m / 100)-th smallest (rule M11); plus the
+ * counters UPDATESTATS keeps.  out: host, [R].  Synchronises. */
 int  ub_stats(ub_sim*, ub_replica_stats* out);
 
 /* Per-request results, each [R][max_requests] (nullable): first / last token time (us, -1 = none yet),
@@ -154,12 +161,38 @@ int  ub_tbt_hist(ub_sim*, uint32_t replica, uint32_t* hist);
 int  ub_debug_get_state(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t* id, uint32_t* d,
                         uint32_t* cached, uint32_t* flags, int64_t* clock_us);
 
+/* Flag bits of ub_debug_get_state / ub_debug_set_state (the `flags` word of a window record). */
+enum { UB_F_RESIDENT = 1u,        /* KV on the device */
+       UB_F_SWAPPED  = 2u,        /* KV in the host swap pool */
+       UB_F_EMITPREV = 4u,        /* emitted a token in the last executed iteration (its t_last is the replica clock) */
+       UB_F_DIRTY    = 8u,        /* (resident, Eq. 8 bin, class) -- the inputs of its key -- changed in the last executed
+                                     iteration: the only requests that may be out of place in the stored order */
+       UB_F_ADMITNOW = 16u,       /* admitted in the last executed iteration */
+       UB_F_KLASS1   = 32u,       /* was in class 1 (not MemGuard-locked) in the last executed iteration */
+       UB_F_LOCK_SHIFT = 6 };     /* bits 6..31: MemGuard lock bin + 1 (0 = no lock; residents re-lock every iteration, M10) */
+
+/* Kernel-level parity (SURVEY.md Sec. 4 tier T1, Sec. 8(b)): overwrite the state of one unfinished replica so that a
+ * single ub_step runs admit / victim-select / advance (a3..a5) from a state taken from elsewhere, e.g. an oracle
+ * snapshot.  Window of n_active requests in stored order: id (< next_request), d tokens emitted (< D), cached KV
+ * tokens (<= P + d; 0 unless resident or swapped), flags (UB_F_*); each host, [n_active].  The stored order must be
+ * the priority order of the state except for the requests flagged UB_F_DIRTY (flag every request to have the next
+ * iteration sort from scratch).  clock_us: replica clock; next_request: trace cursor (requests below it were
+ * ingested); swap_used_blocks: occupancy of the host swap pool.  Counters, digest and per-request outputs are left
+ * as they are.  UB_EINVAL on an inconsistent record, UB_ESTATE if the replica has finished or the state would leave
+ * it finished.  Synchronises. */
+int  ub_debug_set_state(ub_sim*, uint32_t replica, uint32_t n_active, const uint32_t* id, const uint32_t* d,
+                        const uint32_t* cached, const uint32_t* flags, int64_t clock_us, uint32_t next_request,
+                        uint32_t swap_used_blocks);
+
 /* Kernel-level parity (SURVEY.md Sec. 4 tier T1): the (class, key) the device assigns to every request of a replica's
  * window as it stands now, i.e. as the NEXT iteration would score the requests already in the window (a1, M3-M5, M14)
  * -- computed by the same device function the team kernels use.  id, klass: host [queue_cap] u32; key_us: host
  * [queue_cap] i64 (microseconds, or tokens for SRPT / LAS / SJF / SPF); each nullable; *n_active receives the count.
  * Entries come in stored (last priority) order.  Synchronises. */
 int  ub_debug_keys(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us);
+/* The same through the streaming kernel's own scorer (the one bench.py times; FCFS / BOOST with the unified signal
+ * and the geometric quantiser, else UB_EINVAL): pi = a - b_gamma(w_hat) - delta [resident] (Eq. 7). */
+int  ub_debug_keys_stream(ub_sim*, uint32_t replica, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us);
 
 /* Timing of the step kernel launches issued by the LAST ub_step / ub_run call, measured with CUDA events on
  * the borrowed stream: total milliseconds and launch count.  Synchronises. */

@@ -57,7 +57,7 @@ class UbGammaAda(C.Structure):
 EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_step", "ub_run", "ub_stats",
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
            "ub_last_step_timing", "ub_set_iters_per_launch", "ub_set_gamma_ada", "ub_gamma_state", "ub_gamma_grid",
-           "ub_percentile_curve", "ub_slo_attainment", "ub_debug_keys",
+           "ub_percentile_curve", "ub_slo_attainment", "ub_debug_keys", "ub_debug_keys_stream", "ub_debug_set_state",
            "ub_strerror")
 
 _lib = None
@@ -88,6 +88,8 @@ def lib():
         L.ub_last_step_timing.argtypes = [vp, P(C.c_float), P(U32)]
         L.ub_set_iters_per_launch.argtypes = [vp, U32]
         L.ub_debug_keys.argtypes = [vp, U32, P(U32), vp, vp, vp]
+        L.ub_debug_keys_stream.argtypes = [vp, U32, P(U32), vp, vp, vp]
+        L.ub_debug_set_state.argtypes = [vp, U32, U32, vp, vp, vp, vp, I64, U32, U32]
         L.ub_percentile_curve.argtypes = [vp, U32, vp, U32, vp]
         L.ub_slo_attainment.argtypes = [vp, U32, vp, U32, vp]
         L.ub_set_gamma_ada.argtypes = [vp, P(UbGammaAda), vp]
@@ -252,12 +254,22 @@ class Sim:
     def run(self, max_iters=1 << 40, check=True):
         return ub_run(self._h, max_iters, check)
 
-    def debug_keys(self, r=0):
-        """(id, klass, key) arrays of replica r's window as the next iteration would score it (stored order)."""
+    def debug_keys(self, r=0, stream_scorer=False):
+        """(id, klass, key) arrays of replica r's window as the next iteration would score it (stored order);
+        stream_scorer: through the streaming kernel's own scorer (ub_debug_keys_stream)."""
         n = U32(0)
         ids = np.zeros(self.Q, np.uint32); kl = np.zeros(self.Q, np.uint32); ky = np.zeros(self.Q, np.int64)
-        _chk(lib().ub_debug_keys(self._h, int(r), C.byref(n), ids.ctypes.data, kl.ctypes.data, ky.ctypes.data))
+        fn = lib().ub_debug_keys_stream if stream_scorer else lib().ub_debug_keys
+        _chk(fn(self._h, int(r), C.byref(n), ids.ctypes.data, kl.ctypes.data, ky.ctypes.data))
         return ids[:n.value], kl[:n.value], ky[:n.value]
+
+    def debug_set_state(self, r, ids, d, cached, flags, clock_us, next_request, swap_used_blocks=0):
+        """ub_debug_set_state: overwrite replica r's window (stored order), clock, trace cursor and swap occupancy."""
+        a = [np.ascontiguousarray(x, np.uint32) for x in (ids, d, cached, flags)]
+        n = len(a[0])
+        assert all(len(x) == n for x in a)
+        _chk(lib().ub_debug_set_state(self._h, int(r), n, *[x.ctypes.data for x in a], int(clock_us), int(next_request),
+                                      int(swap_used_blocks)))
 
     def percentile_curve(self, which, permille):
         """[R][n] int64 microseconds: nearest-rank percentiles of TTFT (which=0) / TTLT (1) at per-mille points."""

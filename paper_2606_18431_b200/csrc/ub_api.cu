@@ -600,16 +600,21 @@ int ub_per_request(ub_sim* s, int64_t* tf, int64_t* tl, uint32_t* ne, uint32_t* 
   if (tf) CK(cudaMemcpyAsync(tf, s->d_tfirst, tot * 8, kind, s->stream));
   if (tl) CK(cudaMemcpyAsync(tl, s->d_tlast, tot * 8, kind, s->stream));
   if (neu) CK(cudaMemcpyAsync(neu, s->d_neu, tot * 4, kind, s->stream));
-  if (ne) {
+  if (ne) {                                        // bit 31 of the stored word is the completion marker: masked on the device
     if (on_device) {
       k_mask_done<<<148 * 8, 256, 0, s->stream>>>(s->d_ne, ne, tot);
     } else {
-      CK(cudaMemcpyAsync(ne, s->d_ne, tot * 4, kind, s->stream));
+      uint32_t* tmp = nullptr;
+      int rc = dmalloc(&tmp, tot); if (rc) return rc;
+      k_mask_done<<<148 * 8, 256, 0, s->stream>>>(s->d_ne, tmp, tot);
+      cudaError_t e = cudaMemcpyAsync(ne, tmp, tot * 4, kind, s->stream);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+      cudaFree(tmp);
+      if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
     }
   }
   CK(cudaStreamSynchronize(s->stream));
   CK(cudaGetLastError());
-  if (ne && !on_device) for (size_t i = 0; i < tot; i++) ne[i] &= 0x7FFFFFFFu;   // bit 31 is the completion marker
   return UB_OK;
 }
 
@@ -657,9 +662,15 @@ __global__ void k_debug_keys(SimDev s, uint32_t r, uint32_t n, uint32_t* id, uns
   }
 }
 
-int ub_debug_keys(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us) {
+static int debug_keys_impl(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us,
+                           bool stream_scorer) {
   if (!s || r >= s->cfg.n_replicas) return UB_EINVAL;
   if (!s->have_reps) return UB_ESTATE;
+  if (stream_scorer) {                             // the streaming kernel covers FCFS / BOOST with the paper's signal and quantiser
+    const ub_replica& q = s->h_reps[r];
+    if (!(q.policy == UB_FCFS || q.policy == UB_BOOST) || q.signal_mode != UB_SIG_UNIFIED || q.quant_mode != UB_Q_GEOMETRIC)
+      return UB_EINVAL;
+  }
   if (set_dev(s)) return UB_ECUDA;
   Hdr h;
   CK(cudaMemcpyAsync(&h, s->d_hdr + r, sizeof(Hdr), cudaMemcpyDeviceToHost, s->stream));
@@ -670,7 +681,8 @@ int ub_debug_keys(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint3
   uint32_t* d_id = nullptr; unsigned long long* d_key = nullptr;
   int rc = UB_OK;
   if ((rc = dmalloc(&d_id, n)) || (rc = dmalloc(&d_key, n))) { cudaFree(d_id); cudaFree(d_key); return rc; }
-  k_debug_keys<<<(n + 127) / 128, 128, 0, s->stream>>>(s->dev, r, n, d_id, d_key);
+  if (stream_scorer) launch_debug_keys_stream(s->dev, r, n, d_id, d_key, s->stream);
+  else k_debug_keys<<<(n + 127) / 128, 128, 0, s->stream>>>(s->dev, r, n, d_id, d_key);
   std::vector<uint32_t> hid(n); std::vector<unsigned long long> hk(n);
   cudaError_t e = cudaMemcpyAsync(hid.data(), d_id, n * 4, cudaMemcpyDeviceToHost, s->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(hk.data(), d_key, n * 8, cudaMemcpyDeviceToHost, s->stream);
@@ -684,6 +696,13 @@ int ub_debug_keys(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint3
     if (key_us) key_us[i] = (int64_t)(hk[i] & ~(1ull << 63)) - kKeyBias;
   }
   return UB_OK;
+}
+
+int ub_debug_keys(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us) {
+  return debug_keys_impl(s, r, n_active, id, klass, key_us, false);
+}
+int ub_debug_keys_stream(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint32_t* klass, int64_t* key_us) {
+  return debug_keys_impl(s, r, n_active, id, klass, key_us, true);
 }
 
 int ub_debug_get_state(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, uint32_t* d, uint32_t* cached,
@@ -709,4 +728,73 @@ int ub_debug_get_state(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* id, 
     if (flags) flags[i] = e[i].flags;
   }
   return UB_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- ub_debug_set_state
+// err: 0 ok, 1 bad request id / counters, 2 replica already finished or would be left finished
+__global__ void k_set_state(SimDev s, uint32_t r, uint32_t n, const uint32_t* id, const uint32_t* d, const uint32_t* cached,
+                            const uint32_t* flags, int64_t clock, uint32_t next, uint32_t swap_used, int* err) {
+  Hdr& h = s.hdr[r];
+  const RepPar par = h.par;
+  const uint32_t nreq = s.n_req[par.trace_id];
+  const Rec0* TR = s.TR + (size_t)par.trace_id * s.N;
+  __shared__ int bad;
+  if (threadIdx.x == 0) {
+    bad = 0;
+    if (next > nreq || (n == 0 && next >= nreq)) bad = 2;
+    if (h.n_active == 0 && h.a_next == kNever) bad = 2;               // counted as finished already (count[5])
+  }
+  __syncthreads();
+  for (uint32_t p = threadIdx.x; p < n && !bad; p += blockDim.x) {
+    const uint32_t i = id[p];
+    if (i >= next) { atomicExch(&bad, 1); break; }
+    const Rec0 q = TR[i];
+    const uint32_t f = flags[p];
+    if (d[p] >= q.D || cached[p] > q.P + d[p] || ((f & F_RESIDENT) && (f & F_SWAPPED)) ||
+        (!(f & (F_RESIDENT | F_SWAPPED)) && cached[p] != 0u)) { atomicExch(&bad, 1); break; }
+  }
+  __syncthreads();
+  if (bad) { if (threadIdx.x == 0) *err = bad; return; }
+  for (uint32_t p = threadIdx.x; p < n; p += blockDim.x) {
+    Rec1 q1; q1.id = id[p]; q1.d = d[p]; q1.cached = cached[p]; q1.flags = flags[p];
+    s.E0[(size_t)r * s.Q + p] = TR[q1.id];
+    s.E1[(size_t)r * s.Q + p] = q1;
+  }
+  if (threadIdx.x == 0) {
+    h.t = clock;
+    h.a_next = next < nreq ? TR[next].a : kNever;
+    h.n_active = n; h.next = next; h.swap_used = swap_used; h.todo = 0; h.done = 0;
+    if (n > h.peak_active) h.peak_active = n;
+    uint32_t cnt = 0;                                                 // the streaming kernel's dirty list
+    for (uint32_t p = 0; p < n; p++)
+      if (flags[p] & F_DIRTY) { if (cnt < kDirtyMax) h.dl[cnt] = (uint16_t)p; cnt++; }
+    h.n_dirty = cnt > kDirtyMax ? kDirtyMax + 1u : cnt;
+  }
+}
+
+int ub_debug_set_state(ub_sim* s, uint32_t r, uint32_t n, const uint32_t* id, const uint32_t* d, const uint32_t* cached,
+                       const uint32_t* flags, int64_t clock_us, uint32_t next_request, uint32_t swap_used_blocks) {
+  if (!s || r >= s->cfg.n_replicas || n > s->cfg.queue_cap || (n && (!id || !d || !cached || !flags)) || clock_us < 0 ||
+      swap_used_blocks > s->cfg.swap_pool_blocks)
+    return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  uint32_t* dv = nullptr;
+  int rc = dmalloc(&dv, 4 * (size_t)n + 1); if (rc) return rc;
+  cudaError_t e = cudaSuccess;
+  const uint32_t* src[4] = {id, d, cached, flags};
+  for (int k = 0; k < 4 && e == cudaSuccess && n; k++)
+    e = cudaMemcpyAsync(dv + (size_t)k * n, src[k], (size_t)n * 4, cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(dv + 4 * (size_t)n, 0, 4, s->stream);
+  int herr = 0;
+  if (e == cudaSuccess) {
+    k_set_state<<<1, 256, 0, s->stream>>>(s->dev, r, n, dv, dv + n, dv + 2 * (size_t)n, dv + 3 * (size_t)n, clock_us,
+                                          next_request, swap_used_blocks, reinterpret_cast<int*>(dv + 4 * (size_t)n));
+    e = cudaMemcpyAsync(&herr, dv + 4 * (size_t)n, 4, cudaMemcpyDeviceToHost, s->stream);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(dv);
+  if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  return herr == 0 ? UB_OK : (herr == 2 ? UB_ESTATE : UB_EINVAL);
 }

@@ -319,7 +319,5 @@ void launch_slo_count(const SimDev& s, uint32_t which, uint32_t n, const int64_t
   k_slo_count<<<s.R, kStatThreads, 0, st>>>(s, which, n, thr, out);
 }
 
-size_t stats_smem_bytes(uint32_t) { return 0; }
-int stats_configure(uint32_t) { return 0; }
 
 }  // namespace ub

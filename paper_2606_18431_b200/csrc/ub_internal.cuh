@@ -99,9 +99,9 @@ void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iter
                  uint32_t tick, cudaStream_t st);
 void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, cudaStream_t st);
 void launch_stream(const struct StepArgs& A, cudaStream_t st);    // ub_stream.cu
+void launch_debug_keys_stream(const SimDev& s, uint32_t r, uint32_t n, uint32_t* id, unsigned long long* okey, cudaStream_t st);
 void launch_gamma_ada(const SimDev& s, uint32_t rbeg, uint32_t rend, cudaStream_t st);   // ub_aux.cu
 void launch_ada_init(const SimDev& s, cudaStream_t st);
-size_t step_smem_bytes(uint32_t Q);
 int  step_configure(uint32_t Q);
 void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
                           uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st);
@@ -115,7 +115,5 @@ void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st);
 void launch_percentile_curve(const SimDev& s, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out,
                              cudaStream_t st);
 void launch_slo_count(const SimDev& s, uint32_t which, uint32_t n, const int64_t* thr, uint32_t* out, cudaStream_t st);
-size_t stats_smem_bytes(uint32_t N);
-int  stats_configure(uint32_t N);
 
 }  // namespace ub

@@ -686,8 +686,6 @@ __global__ void __launch_bounds__(32 * WARPS * TEAMS) k_step(const StepArgs A, c
 constexpr int kES = 4, kEM = 4, kEL = 8;         // requests per thread: S 1 warp x 4 = 128, M 4 x 4 = 512, L 8 x 8 = 2048
 constexpr int kTeamsS = 4;
 
-size_t step_smem_bytes(uint32_t) { return TeamSmem<8, kEL>::BYTES; }
-
 int step_configure(uint32_t) {
   cudaError_t e = cudaFuncSetAttribute(k_step<8, kEL, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        (int)TeamSmem<8, kEL>::BYTES);

@@ -783,6 +783,27 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 #undef UB_DELTA
 }
 
+// ub_debug_keys_stream: the (class, key) this file's own scorer -- score(), the one the streaming kernel runs -- gives
+// every request of one replica's window as it stands (kernel-level parity of a1, M3-M5); one warp, 32 records a time
+__global__ void k_debug_keys_stream(const SimDev s, const uint32_t r, const uint32_t n, uint32_t* id, unsigned long long* okey) {
+  const int lane = threadIdx.x & 31;
+  const RepPar par = s.hdr[r].par;
+  int64_t lutv = 0;
+  if (par.policy == 2) lutv = __ldg(s.lut + par.lut_off + (size_t)s.hdr[r].level * 64u + lane);
+  for (uint32_t base = 0; base < n; base += 32u) {
+    const uint32_t p = base + (uint32_t)lane;
+    Rec0 q0; Rec1 q1;
+    q0.a = 0; q0.P = 1; q0.D = 1; q1.id = 0; q1.d = 0; q1.cached = 0; q1.flags = 0;
+    if (p < n) { q0 = s.E0[(size_t)r * s.Q + p]; q1 = s.E1[(size_t)r * s.Q + p]; }
+    uint64_t key; uint32_t bin;
+    score(q0, q1, s.k, lutv, par.delta, par.guard != 0, key, bin);
+    if (p < n) { id[p] = q1.id; okey[p] = key; }
+  }
+}
+void launch_debug_keys_stream(const SimDev& s, uint32_t r, uint32_t n, uint32_t* id, unsigned long long* okey, cudaStream_t st) {
+  k_debug_keys_stream<<<1, 32, 0, st>>>(s, r, n, id, okey);
+}
+
 // persistent grid: every warp takes replicas until none is left
 template <bool ADA, bool MULTI> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
   StepArgs A = A0;
