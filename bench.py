@@ -1,25 +1,32 @@
 #!/usr/bin/env python
 """bench.py -- request-steps scheduled per second on B200 and fraction of the HBM roofline.
 
-Workload (BASELINE.json configs[4], the largest single-GPU configuration, "config5"): 65536 replicas x 8192
-requests, 50/50 chat/reasoning mix, Poisson arrivals at 95 % load, KV capacity 16384 blocks, queue cap 2048,
-BOOST gamma = 0.3, swap-vs-recompute preemption; seeded synthetic traces (workloads.config5).
+Workload of the headline line (BASELINE.json configs[4], the largest single-GPU configuration, "config5"): 65536
+replicas x 8192 requests, 50/50 chat/reasoning mix, Poisson arrivals at 95 % load, KV capacity 16384 blocks, queue cap
+2048, BOOST gamma = 0.3, swap-vs-recompute preemption; seeded synthetic traces (workloads.config5).
 
-A "step" is one ub_step(h, ITERS) call: every replica advances ITERS scheduler iterations, each iteration one
-launch of the streaming step kernel ub::k_stream per half of the replicas (all of a0..a5: the replica's window goes
-HBM -> SM -> HBM once); what it queues for the team kernels (nothing in this config) runs once per ub_step call.  Before the timed
-region every replica is advanced SPINUP iterations (not timed, default 65536 = the middle of the ~1.4e5
-iterations a config-5 replica runs) so that the queues are in their loaded regime.  The timed region is K steps on
-the device (CUDA events, barrier + synchronize on both sides, max over ranks).  The windows read per launch
-(~0.4 GB) are larger than L2 (126 MB), so no explicit flush is needed.
+A "step" is one ub_step(h, ITERS) call: every replica advances ITERS scheduler iterations, each iteration one launch of
+the streaming step kernel ub::k_stream per half of the replicas (all of a0..a5: the replica's window goes HBM -> SM ->
+HBM once); what it queues for the team kernels (nothing in this config) runs once per ub_step call.  Before the timed
+region every replica is advanced SPINUP iterations (not timed, default 65536 = the middle of the ~1.4e5 iterations a
+config-5 replica runs) so that the queues are in their loaded regime.  The timed region is K steps on the device (CUDA
+events, barrier + synchronize on both sides, max over ranks).  The windows read per launch (~0.4 GB) are larger than L2
+(126 MB), so no explicit flush is needed.
+
+Beside the headline the line carries (extra keys): the same job from the first arrival to the last completion
+(`whole_job`), the device-resident percentile reduction timed at full size (`stats`), the resident-state mode, and --
+on one GPU -- the chat-heavy (config 2) and reasoning-heavy (config 3) workloads of BASELINE.json run as whole jobs
+(`workloads`), the oracle on one host core and on all of them (`cpu_baseline`).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -34,11 +41,14 @@ if ROOT not in sys.path:
 from paper_2606_18431_b200 import workloads as W  # noqa: E402
 
 RESIDENT_IPL = 16
-KERNELS_PER_ROUND = 2                # a round = two halves on two streams, one ub::k_stream launch each (team kernels run once per ub_step)
-TRAFFIC_BYTES_PER_LAUNCH = 463.3e6   # dram read+write bytes of the two ub::k_stream launches of one round, profiles/r01g_stream.md
-ALG_BYTES_PER_REQUEST_STEP = 40      # DESIGN.md Sec. 6: read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
+ALG_BYTES_PER_REQUEST_STEP = 40      # DESIGN.md Sec. 7: read a,P,D,d,cached,flags (28 B) + write d,cached,flags (12 B)
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_stream_traffic.csv")   # written from the ncu --set full capture
 METRIC = "request-steps scheduled/sec"
 UNIT = "request-steps/s"
+COLS = ["iterations", "request_steps", "n_completed", "evict_recompute", "evict_swap", "swapins", "tokens_lost",
+        "tokens_emitted", "prefill_tokens", "decode_seqs", "t_end_us", "peak_active", "done", "swap_used"]
+COL = {name: i for i, name in enumerate(COLS)}
+TTLT_P99_COL = len(COLS) + 3 + 2       # ttft_us[3], then ttlt_us[2]
 
 
 def parse():
@@ -52,8 +62,9 @@ def parse():
     ap.add_argument("--replicas", type=int, default=65536, help="replicas per GPU (config5: 65536)")
     ap.add_argument("--requests", type=int, default=8192)
     ap.add_argument("--iters-per-launch", type=int, default=1)
-    ap.add_argument("--cpu-sample", type=int, default=64, help="replicas the oracle baseline runs")
+    ap.add_argument("--cpu-sample", type=int, default=64, help="replicas the one-core oracle baseline runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="headline only: no whole job, no config 2 / 3 (profiling runs)")
     return ap.parse_args()
 
 
@@ -65,6 +76,18 @@ def peaks():
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def profiled_traffic():
+    """DRAM read + write bytes of the k_stream launches of one round, from the committed ncu capture of this kernel
+    (profiles/r02_stream_traffic.csv: one row per launch of the round); None if the file is absent."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            rows = [r for r in csv.DictReader(l for l in f if not l.startswith("#"))]
+        return float(sum(float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]) for r in rows)), \
+            os.path.relpath(TRAFFIC_CSV, ROOT)
+    except Exception:
+        return None, None
 
 
 class ClockSampler:
@@ -110,10 +133,13 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_rate(wl, replica_ids, n_iters):
-    """The oracle as it stands, single thread, on a bounded sample of the same workload."""
+# ---------------------------------------------------------------------------------------------- the oracle legs
+
+def _oracle_job(job):
+    """(request-steps, seconds) of the oracle as it stands, single thread, on the given replicas of config 5."""
+    n_seeds, n_requests, ids, n_iters = job
     from oracle import oracle as O
-    sub = wl.select(replica_ids)
+    sub = W.config5(n_seeds=n_seeds, n_requests=n_requests).select(ids)
     o = O.OracleSim(sub.sim, sub.replicas, sub.traces())
     t0 = time.perf_counter()
     o.step(n_iters)
@@ -121,6 +147,29 @@ def oracle_rate(wl, replica_ids, n_iters):
     rs = sum(s["request_steps"] for s in o.stats())
     o.close()
     return rs, dt
+
+
+def cpu_baselines(R, N, n_iters, sample):
+    """The oracle on one host core, and on all of them (one process per core, each its own replicas)."""
+    import multiprocessing as mp
+    ids = list(range(0, R, max(1, R // sample)))[:sample]
+    rs1, dt1 = _oracle_job((R, N, ids, n_iters))
+    out = {"value": rs1 / dt1, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"{len(ids)} of {R} replicas of config5 for the same {n_iters} iterations ({dt1:.1f} s)"}
+    nproc = os.cpu_count() or 1
+    per = max(2, sample // 4)
+    pool_ids = [r % R for r in range(1, 1 + nproc * per * 7, 7)]
+    jobs = [(R, N, pool_ids[i * per:(i + 1) * per], n_iters) for i in range(nproc)]
+    t0 = time.perf_counter()
+    with mp.get_context("spawn").Pool(nproc) as pool:
+        res = pool.map(_oracle_job, jobs)
+    wall = time.perf_counter() - t0
+    busy = max(dt for _, dt in res)
+    out["all_cores"] = {"value": sum(rs for rs, _ in res) / busy, "unit": UNIT, "cores": nproc, "nproc": nproc,
+                        "kind": "oracle, one process per core",
+                        "sample": f"{per} replicas per process x {nproc} processes for the same {n_iters} iterations "
+                                  f"(slowest process {busy:.1f} s, wall with start-up {wall:.1f} s)"}
+    return out
 
 
 def run_reference(args):
@@ -133,7 +182,6 @@ def run_reference(args):
     sub = wl.select(ids)
     o = O.OracleSim(sub.sim, sub.replicas, sub.traces())
     o.step(args.spinup)                                   # same populated-queue regime as the CUDA arm
-    rs0 = sum(s["request_steps"] for s in o.stats())
     for _ in range(args.warmup):
         o.step(args.iters)
     rs1 = sum(s["request_steps"] for s in o.stats())
@@ -143,7 +191,8 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     rs2 = sum(s["request_steps"] for s in o.stats())
     val = (rs2 - rs1) / dt
-    sample = f"{len(ids)} of {args.replicas} replicas of config5, {args.steps} steps x {args.iters} iterations after {args.spinup} spin-up iterations"
+    sample = (f"{len(ids)} of {args.replicas} replicas of config5, {args.steps} steps x {args.iters} iterations after "
+              f"{args.spinup} spin-up iterations")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
@@ -155,33 +204,84 @@ def run_reference(args):
         "gpu_launches": 0,
     }))
     o.close()
-    del rs0
+
+
+# ---------------------------------------------------------------------------------------------- the CUDA arm
+
+def reexec_under_torchrun(args):
+    """`python bench.py --gpus N` outside torchrun: launch N ranks of this script (one per GPU) and become them."""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
+def stats_table(B, sim, R):
+    st = sim.stats_raw()                                             # device percentile reduction + D2H
+    words = B.C.sizeof(B.UbReplicaStats) // 8
+    return np.frombuffer(st, dtype=np.int64).reshape(R, words).copy()
+
+
+def whole_job(B, wl, traces, stream, peak, label):
+    """One workload from the first arrival to the last completion through ub_run; request-steps / device time of the
+    step launches (CUDA events inside ub_run), the 40-byte roofline fraction and the mean window size."""
+    R = int(wl.sim["n_replicas"])
+    sim = B.Sim(wl.sim, wl.replicas, traces, stream=stream)
+    t0 = time.perf_counter()
+    issued = sim.run()
+    wall = time.perf_counter() - t0
+    ms, launches = sim.last_step_timing()
+    t1 = time.perf_counter()
+    st = stats_table(B, sim, R)
+    t_stats = time.perf_counter() - t1
+    rs = int(st[:, COL["request_steps"]].sum()); its = int(st[:, COL["iterations"]].sum())
+    sim.close()
+    return {"workload": label, "replicas": R, "value": rs / (ms * 1e-3), "unit": UNIT,
+            "roofline_frac": rs * ALG_BYTES_PER_REQUEST_STEP / (ms * 1e-3) / 1e9 / peak,
+            "request_steps": rs, "device_ms": ms, "wall_s": wall, "iterations_issued": int(issued),
+            "iterations_executed_max": int(st[:, COL["iterations"]].max()), "rounds_launched": int(launches),
+            "mean_window": rs / max(1, its), "ub_stats_s": t_stats,
+            "completed": int(st[:, COL["n_completed"]].sum())}
 
 
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        reexec_under_torchrun(args)
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus != world:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}")
+
+    # ---- synthetic traces first (the generator forks worker processes: before CUDA / NCCL are initialised).
+    # Replicas are independent units, sharded over ranks by seed (weak scaling).
+    from paper_2606_18431_b200 import sharding as SH
+    R, N = args.replicas, args.requests
+    wl = SH.shard_workload(W.config5, rank, world, R, N)
+    t_gen = time.perf_counter()
+    nw = max(1, min(32, (os.cpu_count() or 1) // max(1, world)))
+    a, p, d, n = wl.traces(workers=nw)
+    t_gen = time.perf_counter() - t_gen
+    # (on one GPU also the chat-heavy and reasoning-heavy workloads north_star names, run as whole jobs at the end)
+    side = []
+    if world == 1 and not args.no_extras:
+        for mk, label in ((W.config2, "config2: chat-heavy, 1024 seeds x {FCFS, SRPT, BOOST}"),
+                          (W.config3, "config3: reasoning-heavy, 4096 replicas, MMPP-2 arrivals, swap-vs-recompute")):
+            w2 = mk()
+            side.append((w2, w2.traces(workers=nw), label))
 
     import torch
     import torch.distributed as dist
     from paper_2606_18431_b200 import binding as B
-    from paper_2606_18431_b200 import sharding as SH
-
-    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    # ---- synthetic traces: replicas are independent units, sharded over ranks by seed (weak scaling)
-    R, N = args.replicas, args.requests
-    wl = SH.shard_workload(W.config5, rank, world, R, N)
-    t_gen = time.perf_counter()
-    a, p, d, n = wl.traces(workers=max(1, min(32, (os.cpu_count() or 1) // max(1, world))))
-    t_gen = time.perf_counter() - t_gen
     pin = [torch.from_numpy(x).pin_memory() for x in (a, p, d)]       # e2e copies from pinned host memory
     a, p, d = [x.numpy() for x in pin]
     h2d_bytes = a.nbytes + p.nbytes + d.nbytes + n.nbytes
@@ -193,20 +293,14 @@ def main():
     t_e2e0 = time.perf_counter()
     h = B.ub_create(B.make_config(wl.sim, args.iters_per_launch, local, stream))
     B.ub_load_trace(h, a, p, d, n)                                   # host -> device inside the e2e region
-    B.ub_set_replicas(h, B.make_replicas(wl.replicas, R))
+    reps = B.make_replicas(wl.replicas, R)
+    B.ub_set_replicas(h, reps)
     sim = B.Sim.__new__(B.Sim); sim._h, sim.R, sim.N, sim.Q = h, R, N, int(wl.sim["queue_cap"])
 
     B.ub_step(h, args.spinup)                                        # populate the queues (untimed)
     for _ in range(args.warmup):
         B.ub_step(h, args.iters)
-    def stats_table():
-        st = sim.stats_raw()                                         # device percentile reduction + D2H
-        words = B.C.sizeof(B.UbReplicaStats) // 8
-        return np.frombuffer(st, dtype=np.int64).reshape(R, words).copy()
-    COL = {name: i for i, name in enumerate(
-        ["iterations", "request_steps", "n_completed", "evict_recompute", "evict_swap", "swapins", "tokens_lost",
-         "tokens_emitted", "prefill_tokens", "decode_seqs", "t_end_us", "peak_active", "done", "swap_used"])}
-    st1 = stats_table()
+    st1 = stats_table(B, sim, R)
     rs1 = int(st1[:, COL["request_steps"]].sum()); it1 = int(st1[:, COL["iterations"]].max())
     live1 = int((st1[:, COL["done"]] == 0).sum())
 
@@ -225,14 +319,15 @@ def main():
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
 
-    st2 = stats_table()
+    st2 = stats_table(B, sim, R)
     t_e2e = time.perf_counter() - t_e2e0
+    rs2 = int(st2[:, COL["request_steps"]].sum())
 
     # resident-state mode, reported separately: 16 iterations per launch, a warp advances its
     # replica 16 iterations in a row and the window is re-read from L2; same schedule, fewer HBM bytes
     B.ub_set_iters_per_launch(h, RESIDENT_IPL)
     B.ub_step(h, args.iters)
-    st3 = stats_table()
+    st3 = stats_table(B, sim, R)
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record()
     for _ in range(args.steps):
@@ -240,17 +335,50 @@ def main():
     f1.record()
     torch.cuda.synchronize()
     ms_res = f0.elapsed_time(f1)
-    st4 = stats_table()
+    st4 = stats_table(B, sim, R)
     rs_res = int(st4[:, COL["request_steps"]].sum()) - int(st3[:, COL["request_steps"]].sum())
     B.ub_set_iters_per_launch(h, args.iters_per_launch)
-    rs2 = int(st2[:, COL["request_steps"]].sum())
+
     d2h_bytes = R * (B.C.sizeof(B.UbReplicaStats))
-    ttlt_p99_us = st2[:, 14 + 3 + 2][st2[:, COL["n_completed"]] > 0]          # ttlt_us[2]
+    ttlt_p99_us = st2[:, TTLT_P99_COL][st2[:, COL["n_completed"]] > 0]
     p99 = float(np.median(ttlt_p99_us)) * 1e-6 if ttlt_p99_us.size else 0.0
-    rounds = args.steps * ((args.iters + max(1, args.iters_per_launch) - 1) // max(1, args.iters_per_launch))
-    launches = rounds * KERNELS_PER_ROUND
+    ipl = max(1, args.iters_per_launch)
+    rounds = args.steps * ((args.iters + ipl - 1) // ipl)
+    nsplit = 2 if R >= 8192 else 1
+    # kernels of this library launched inside the timed region: per round one k_stream per half; per ub_step call the
+    # hand-over flush (one k_step<8,8,1> per half in an all-streaming job; plus one 16-byte memset per half)
+    launches = rounds * nsplit + args.steps * nsplit
+    steps_in_job = args.spinup / max(1, args.iters) + args.warmup + args.steps
+
+    # ---- the same job from the first arrival to the last completion (ub_set_replicas rewinds it), and the percentile
+    # reduction at full size behind it
+    extras = {}
+    if not args.no_extras:
+        B.ub_set_replicas(h, reps)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        issued = B.ub_run(h)
+        wall = time.perf_counter() - t0
+        ms_job, rounds_job = B.ub_last_step_timing(h)
+        t0 = time.perf_counter()
+        stj = stats_table(B, sim, R)
+        t_stats = time.perf_counter() - t0
+        rs_job = int(stj[:, COL["request_steps"]].sum())
+        extras["whole_job"] = {
+            "value": rs_job / (ms_job * 1e-3) * world, "unit": UNIT, "request_steps_per_gpu": rs_job,
+            "device_s": ms_job * 1e-3, "wall_s": wall, "iterations_issued": int(issued),
+            "iterations_executed_max": int(stj[:, COL["iterations"]].max()), "rounds_launched": int(rounds_job),
+            "mean_window": rs_job / max(1, int(stj[:, COL["iterations"]].sum())),
+            "completed_per_gpu": int(stj[:, COL["n_completed"]].sum()),
+            "note": "config5 from the first arrival to the last completion through ub_run, one iteration per launch: "
+                    "ramp-up with small windows, the loaded middle, the tail with few live replicas; per-rank value x ranks"}
+        extras["stats"] = {"ub_stats_s": t_stats, "requests_reduced": int(stj[:, COL["n_completed"]].sum()),
+                           "note": "ub_stats at full size: k_stats (6 exact nearest-rank selections per replica over its "
+                                   "completed requests + TBT histogram percentiles) + D2H of R structs + host conversion"}
 
     rs_timed, rs_all, ms, t_e2e = SH.aggregate(rs2 - rs1, rs2, ms, t_e2e, "cuda", world)
+    job_stats = SH.gather_replica_stats(st2[:, [COL["request_steps"], COL["n_completed"], TTLT_P99_COL]], "cuda", world)
+    sim.close()
 
     if rank == 0:
         peak, peak_src = peaks()
@@ -258,40 +386,47 @@ def main():
         per_gpu_bytes = (rs2 - rs1) * ALG_BYTES_PER_REQUEST_STEP
         ach = per_gpu_bytes / (ms * 1e-3) / 1e9
         n_mean = (rs2 - rs1) / max(1, (args.steps * args.iters)) / max(1, live1)
+        traffic, traffic_src = profiled_traffic()
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / max(1, args.steps), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
             "config": {"workload": "config5: 65536 replicas x 8192 requests, 50/50 chat/reasoning, 95% load, KV 16384 blocks, queue cap 2048",
                        "replicas_per_gpu": R, "requests": N, "iters_per_step": args.iters,
-                       "iters_per_launch": max(1, args.iters_per_launch), "spinup_iters": args.spinup,
+                       "iters_per_launch": ipl, "spinup_iters": args.spinup,
                        "mean_active_per_live_replica": n_mean, "live_replicas": live1,
                        "iterations_before_timed": int(it1), "l2": "inputs larger than L2 (no flush)",
-                       "trace_generation_s": t_gen, "median_p99_ttlt_s": p99},
+                       "trace_generation_s": t_gen, "median_p99_ttlt_s": p99,
+                       "job_replicas_gathered": int(job_stats.shape[0])},
             "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                         "traffic": TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src, "kernel": "ub::k_stream",
+                         "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                         "kernel": "ub::k_stream<false,false>",
                          "alg_bytes_per_request_step": ALG_BYTES_PER_REQUEST_STEP,
                          "request_steps_per_launch": (rs2 - rs1) / max(1, rounds),
                          "avg_launch_ms": ms / max(1, rounds),
                          "note": "a round = every live replica advanced one iteration = two overlapping k_stream launches "
                                  "(one half of the replicas each, on two streams); the team kernels run once per ub_step; "
                                  "avg_launch_ms, request_steps_per_launch and traffic are per round; traffic = dram "
-                                 "read+write bytes of the round's k_stream launches from profiles/ (ncu --set full)"},
-            "e2e": {"value": rs_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": d2h_bytes,
-                    "note": "one job: ub_create + ub_load_trace from pinned host + ub_set_replicas + spin-up + warm-up + timed steps + 2x ub_stats D2H; all request-steps / wall"},
+                                 "read+write bytes of the round's k_stream launches in the committed ncu --set full capture"},
+            "e2e": {"value": rs_all / t_e2e, "unit": UNIT, "h2d_bytes_per_step": h2d_bytes / steps_in_job,
+                    "d2h_bytes_per_step": 2 * d2h_bytes / steps_in_job, "h2d_bytes_per_job": h2d_bytes,
+                    "d2h_bytes_per_job": 2 * d2h_bytes, "steps_in_job": steps_in_job,
+                    "note": "one job through the C-ABI from pinned host buffers: ub_create + ub_load_trace (H2D) + ub_set_replicas "
+                            "+ spin-up + warm-up + timed steps (steps_in_job steps of iters_per_step iterations) + 2x ub_stats "
+                            "(D2H); all request-steps / wall; bytes per step = bytes of the job / steps_in_job"},
             "resident": {"value": rs_res / (ms_res * 1e-3) * world, "unit": UNIT, "iters_per_launch": RESIDENT_IPL,
                          "note": "same K steps with 16 iterations per kernel launch (window re-read from L2, not HBM); "
                                  "per-rank value x ranks; not the roofline path"},
             "gpu_launches": launches, "clocks": clocks,
         }
-        if not args.no_cpu_baseline:
-            ids = list(range(0, R, max(1, R // args.cpu_sample)))[:args.cpu_sample]
+        out.update(extras)
+        if world == 1 and not args.no_extras:
+            # the chat-heavy and reasoning-heavy workloads north_star names, as whole jobs
+            out["workloads"] = [whole_job(B, w2, tr2, stream, peak, label) for w2, tr2, label in side]
+        if not args.no_cpu_baseline and world == 1:
             n_it = args.spinup + (args.warmup + args.steps) * args.iters
-            rs_o, dt_o = oracle_rate(wl, ids, n_it)
-            out["cpu_baseline"] = {"value": rs_o / dt_o, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                   "sample": f"{len(ids)} of {R} replicas of config5 for the same {n_it} iterations ({dt_o:.1f} s)"}
+            out["cpu_baseline"] = cpu_baselines(R, N, n_it, args.cpu_sample)
         print(json.dumps(out))
-    sim.close()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

@@ -73,9 +73,9 @@ typedef struct {
   uint32_t swap_pool_blocks;      /* host swap pool, blocks */
   uint32_t bin_tokens;            /* MemGuard k (Eq. 8) */
   uint32_t tok_us;                /* service us credited per token in the argument of b_gamma (reading G1) */
-  int64_t  c0_us;                 /* iteration cost = c0 + c_prefill_tok * prefill tokens            */
-  int64_t  c_prefill_tok_us;      /*                + c_decode_seq * decode sequences + swap time (M9) */
-  int64_t  c_decode_seq_us;
+  int64_t  c0_us;                 /* iteration cost = c0 + c_prefill_tok * prefill tokens            (<= 2^40) */
+  int64_t  c_prefill_tok_us;      /*                + c_decode_seq * decode sequences + swap time (M9); <= 2^20 */
+  int64_t  c_decode_seq_us;       /* <= 2^30 */
   uint32_t iters_per_launch;      /* scheduler iterations one kernel launch advances; 0 or 1 = one iteration per
                                      launch with the state streamed HBM -> SM -> HBM every iteration */
   int32_t  device;                /* CUDA device ordinal */

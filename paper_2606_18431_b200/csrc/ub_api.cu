@@ -25,6 +25,8 @@ struct ub_sim {
   int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
   uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([5] = finished replicas)
+  uint32_t* d_live; uint32_t* d_livecnt; // ub_run's tail: the unfinished replicas of each part of a round, compacted
+  bool use_list; uint32_t livecnt[ub::kMaxSplit];
   int64_t* d_ada_ring; AdaState* d_ada_state; int64_t* d_ada_grid;   // gamma-Ada (M13), null when off
   std::vector<int64_t> h_ada_grid;
   uint2* d_evbuf;                        // per-iteration event scratch [R][min(M,Q)]
@@ -77,7 +79,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
     return UB_EINVAL;
   // value ranges that keep every device quantity inside u32 / the flags word
   if ((uint64_t)c->kv_blocks * c->block_tokens >= (1ull << 27) || c->bin_tokens >= (1u << 27) ||
-      c->c0_us > (1ll << 40) || c->c_prefill_tok_us > (1ll << 30) || c->c_decode_seq_us > (1ll << 30))
+      c->c0_us > (1ll << 40) || c->c_prefill_tok_us > (1ll << 20) || c->c_decode_seq_us > (1ll << 30))
     return UB_EINVAL;
   if (cudaSetDevice(c->device) != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
   ub_sim* s = new (std::nothrow) ub_sim();
@@ -87,6 +89,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
   s->have_trace = s->have_reps = false;
   s->d_TR = nullptr; s->d_lut = nullptr;
   s->last_ms = 0.f; s->last_launches = 0;
+  s->use_list = false;
   s->nsplit = c->n_replicas >= 8192 ? 2 : 1;          // (measured on config 5: 2 parts 5.9e10, 4 parts 5.5e10 request-steps/s)
   const size_t R = c->n_replicas, Q = c->queue_cap, N = c->max_requests, NT = c->n_traces;
   int rc = UB_OK;
@@ -94,12 +97,12 @@ int ub_create(const ub_config* c, ub_sim** out) {
       (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
-      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_list, 4 * kMaxSplit * R)) || (rc = dmalloc(&s->d_count, 8 * kMaxSplit)) ||
+      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_live, R)) || (rc = dmalloc(&s->d_livecnt, kMaxSplit)) || (rc = dmalloc(&s->d_list, 4 * kMaxSplit * R)) || (rc = dmalloc(&s->d_count, 8 * kMaxSplit)) ||
       (rc = dmalloc(&s->d_evbuf, R * (size_t)(c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap)))) {
     ub_destroy(s);
     return rc;
   }
-  if (cudaMallocHost((void**)&s->h_word, 2 * sizeof(unsigned long long)) != cudaSuccess ||
+  if (cudaMallocHost((void**)&s->h_word, (2 + kMaxSplit) * sizeof(unsigned long long)) != cudaSuccess ||
       cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess ||
       cudaStreamCreateWithFlags(&s->aux[0], cudaStreamNonBlocking) != cudaSuccess ||
       cudaStreamCreateWithFlags(&s->aux[1], cudaStreamNonBlocking) != cudaSuccess ||
@@ -135,7 +138,7 @@ void ub_destroy(ub_sim* s) {
   cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_TR);
   cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
-  cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_evbuf);
+  cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_evbuf); cudaFree(s->d_live); cudaFree(s->d_livecnt);
   cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);
   if (s->h_word) cudaFreeHost(s->h_word);
   if (s->ev0) cudaEventDestroy(s->ev0);
@@ -235,6 +238,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
     any_exact |= (q.quant_mode == UB_Q_EXACT);
   }
   s->have_reps = false;
+  s->use_list = false;                             // (a rewound run: every replica is live again)
   cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);        // adaptation is set per replica table
   s->d_ada_ring = nullptr; s->d_ada_state = nullptr; s->d_ada_grid = nullptr; s->h_ada_grid.clear();
   s->dev.ada_ring = nullptr; s->dev.ada_state = nullptr; s->dev.ada_grid = nullptr;
@@ -323,7 +327,9 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
     for (uint32_t i = 0; i < ns; i++) {
       const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
       if (ada) launch_gamma_ada(s->dev, rb, re, i ? s->aux[i - 1] : s->stream);
-      launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, s->round_no, i ? s->aux[i - 1] : s->stream);
+      const bool lst = s->use_list && !ada;
+      launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, s->round_no,
+                  lst ? s->d_live + rb : nullptr, lst ? s->livecnt[i] : 0u, i ? s->aux[i - 1] : s->stream);
     }
     n_iters -= k; nl++; s->round_no++;
     // what k_stream queued for the team kernels runs at the end of the call (all owed iterations at once); with
@@ -367,15 +373,42 @@ int ub_step(ub_sim* s, uint32_t n_iters, uint64_t* live) {
   return UB_OK;
 }
 
+// The unfinished replicas of every part of a round, compacted on the device; *live = how many.  From then on the
+// streaming kernel visits only these (a finished replica never comes back, so the list stays a superset of the live
+// replicas until it is rebuilt; ub_set_replicas drops it).
+static int compact_live(ub_sim* s, uint64_t* live) {
+  const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
+  const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
+  for (uint32_t i = 0; i < ns; i++) {
+    const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
+    launch_compact_live(s->dev, rb, re, s->d_live + rb, s->d_livecnt + i, s->stream);
+  }
+  uint32_t* hc = reinterpret_cast<uint32_t*>(s->h_word + 2);
+  CK(cudaMemcpyAsync(hc, s->d_livecnt, ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
+  CK(cudaGetLastError());
+  uint64_t tot = 0;
+  for (uint32_t i = 0; i < ns; i++) { s->livecnt[i] = hc[i]; tot += hc[i]; }
+  s->use_list = true;
+  *live = tot;
+  return UB_OK;
+}
+
 int ub_run(ub_sim* s, uint64_t max_iters, uint64_t* iters_done) {
   if (!s) return UB_EINVAL;
   if (!s->have_reps) return UB_ESTATE;
   if (set_dev(s)) return UB_ECUDA;
+  const uint64_t R = s->cfg.n_replicas;
+  const bool ada = s->d_ada_ring != nullptr;
   uint64_t done = 0, live = 1;
   uint32_t total_launches = 0;
   float total_ms = 0.f;
   int rc = read_live(s, &live);
   if (rc) return rc;
+  // While every replica is live the liveness is polled at growing intervals (256 .. 4096 iterations).  Once replicas
+  // start to finish, every poll (512 iterations apart: the overshoot behind the last completion stays small)
+  // compacts the unfinished ones into a list, and the streaming kernel visits only those: the tail of a run, in which
+  // few replicas are still draining their queues, no longer pays for the headers of all the finished ones.
   uint64_t chunk = 256;
   while (live > 0 && done < max_iters) {
     const uint64_t k = (max_iters - done) < chunk ? (max_iters - done) : chunk;
@@ -389,7 +422,11 @@ int ub_run(ub_sim* s, uint64_t max_iters, uint64_t* iters_done) {
     float ms = 0.f;
     CK(cudaEventElapsedTime(&ms, s->ev0, s->ev1));
     total_ms += ms;
-    if (chunk < 4096) chunk *= 2;
+    if (live == R) { if (chunk < 4096) chunk *= 2; }
+    else {
+      chunk = 512;
+      if (!ada && live > 0 && live * 8 < R * 7 && (rc = compact_live(s, &live))) return rc;
+    }
   }
   s->last_ms = total_ms; s->last_launches = total_launches;
   if (iters_done) *iters_done = done;
@@ -440,14 +477,18 @@ int ub_set_gamma_ada(ub_sim* s, const ub_gamma_ada* g, const uint8_t* adaptive) 
   }
   std::vector<int64_t> grid(g->levels);
   for (uint32_t j = 0; j < g->levels; j++) grid[j] = (int64_t)floor(ada_grid_gamma(g, j) * 1e6 + 0.5);
+  // Everything is built in temporaries and committed to the handle only after every allocation and copy has
+  // succeeded; on failure the handle keeps its old (non-adaptive) state.
   // tables of the grid levels, appended to the static ones; adaptive replicas point at them
-  const size_t base = s->h_lut.size();
+  std::vector<int64_t> lut(s->h_lut);
+  const size_t base = lut.size();
   if (base + (size_t)g->levels * 64 >= (1ull << 32)) return UB_ENOMEM;
   for (uint32_t j = 0; j < g->levels; j++)
     for (uint32_t b = 0; b < 64; b++)
-      s->h_lut.push_back(boost_table_entry(ada_grid_gamma(g, j), ldexp((double)c.bin_tokens, (int)b), c.tok_us));
+      lut.push_back(boost_table_entry(ada_grid_gamma(g, j), ldexp((double)c.bin_tokens, (int)b), c.tok_us));
   std::vector<AdaState> st(R);
   std::vector<RepPar> par(R);
+  std::vector<uint32_t> lut_off(s->h_lut_off), lut_nb(s->h_lut_nb);
   CK(cudaMemcpy2D(par.data(), sizeof(RepPar), &s->d_hdr[0].par, sizeof(Hdr), sizeof(RepPar), R, cudaMemcpyDeviceToHost));
   for (size_t r = 0; r < R; r++) {
     memset(&st[r], 0, sizeof(AdaState));
@@ -459,19 +500,38 @@ int ub_set_gamma_ada(ub_sim* s, const ub_gamma_ada* g, const uint8_t* adaptive) 
     while (lvl + 1 < g->levels && grid[lvl + 1] <= gu) lvl++;
     st[r].gamma_u = gu; st[r].level = lvl; st[r].on = 1;
     par[r].lut_off = (uint32_t)base; par[r].lut_nb = 64;
-    s->h_lut_off[r] = (uint32_t)base; s->h_lut_nb[r] = 64;
+    lut_off[r] = (uint32_t)base; lut_nb[r] = 64;
   }
+  int64_t* n_lut = nullptr; int64_t* n_ring = nullptr; AdaState* n_state = nullptr; int64_t* n_grid = nullptr;
   int rc = UB_OK;
-  cudaFree(s->d_lut); s->d_lut = nullptr;
-  if ((rc = dmalloc(&s->d_lut, s->h_lut.size())) || (rc = dmalloc(&s->d_ada_ring, R * (size_t)g->window)) ||
-      (rc = dmalloc(&s->d_ada_state, R)) || (rc = dmalloc(&s->d_ada_grid, (size_t)g->levels)))
+  if ((rc = dmalloc(&n_lut, lut.size())) || (rc = dmalloc(&n_ring, R * (size_t)g->window)) ||
+      (rc = dmalloc(&n_state, R)) || (rc = dmalloc(&n_grid, (size_t)g->levels))) {
+    cudaFree(n_lut); cudaFree(n_ring); cudaFree(n_state); cudaFree(n_grid);
     return rc;
-  CK(cudaMemcpyAsync(s->d_lut, s->h_lut.data(), s->h_lut.size() * 8, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpy2DAsync(&s->d_hdr[0].par, sizeof(Hdr), par.data(), sizeof(RepPar), sizeof(RepPar), R,
-                       cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->d_ada_state, st.data(), R * sizeof(AdaState), cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemcpyAsync(s->d_ada_grid, grid.data(), grid.size() * 8, cudaMemcpyHostToDevice, s->stream));
-  CK(cudaMemsetAsync(s->d_ada_ring, 0, R * (size_t)g->window * 8, s->stream));
+  }
+  // (the parameter records inside the headers are the last thing written: they only take effect with the new table)
+  cudaError_t e = cudaMemcpyAsync(n_lut, lut.data(), lut.size() * 8, cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(n_state, st.data(), R * sizeof(AdaState), cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(n_grid, grid.data(), grid.size() * 8, cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(n_ring, 0, R * (size_t)g->window * 8, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  bool par_touched = false;
+  if (e == cudaSuccess) {
+    par_touched = true;
+    e = cudaMemcpy2DAsync(&s->d_hdr[0].par, sizeof(Hdr), par.data(), sizeof(RepPar), sizeof(RepPar), R,
+                          cudaMemcpyHostToDevice, s->stream);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    if (par_touched) s->have_reps = false;         // the replica table may be half written: ub_set_replicas again
+    cudaFree(n_lut); cudaFree(n_ring); cudaFree(n_state); cudaFree(n_grid);
+    return UB_ECUDA;
+  }
+  // commit
+  cudaFree(s->d_lut);
+  s->d_lut = n_lut; s->d_ada_ring = n_ring; s->d_ada_state = n_state; s->d_ada_grid = n_grid;
+  s->h_lut.swap(lut); s->h_lut_off.swap(lut_off); s->h_lut_nb.swap(lut_nb);
   SimDev& d = s->dev;
   d.lut = s->d_lut; d.ada_ring = s->d_ada_ring; d.ada_state = s->d_ada_state; d.ada_grid = s->d_ada_grid;
   d.ada_W = g->window; d.ada_G = g->levels; d.ada_min = g->min_samples; d.ada_shift = g->beta_shift; d.ada_eps = g->eps_us;
@@ -636,7 +696,15 @@ int ub_boost_lut(ub_sim* s, uint32_t r, int64_t* lut, uint32_t cap, uint32_t* nb
   *nb = n;
   if (lut) {
     const bool boost = s->h_reps[r].policy == UB_BOOST || s->h_reps[r].policy == UB_DISTBOOST;
-    for (uint32_t b = 0; b < n && b < cap; b++) lut[b] = boost ? s->h_lut[s->h_lut_off[r] + b] : 0;
+    size_t off = s->h_lut_off[r];
+    if (s->d_ada_state) {                          // a gamma-Ada replica: the table of the grid level in use
+      if (set_dev(s)) return UB_ECUDA;
+      AdaState st;
+      CK(cudaMemcpyAsync(&st, s->d_ada_state + r, sizeof(AdaState), cudaMemcpyDeviceToHost, s->stream));
+      CK(cudaStreamSynchronize(s->stream));
+      if (st.on) off += (size_t)st.level * 64u;
+    }
+    for (uint32_t b = 0; b < n && b < cap; b++) lut[b] = boost ? s->h_lut[off + b] : 0;
   }
   return UB_OK;
 }

@@ -126,6 +126,26 @@ void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* li
   k_count_live<<<1, 1, 0, st>>>(count, R, live);
 }
 
+// The unfinished replicas of [rbeg, rend), compacted (ub_run's tail: the streaming kernel then visits only these).
+// A replica is finished when its trace is exhausted and nothing is active (M6); finished replicas never come back.
+__global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, uint32_t* out, uint32_t* cnt) {
+  const uint32_t lane = threadIdx.x & 31u;
+  for (uint32_t base = rbeg + (blockIdx.x * blockDim.x + threadIdx.x - lane); base < rend; base += gridDim.x * blockDim.x) {
+    const uint32_t r = base + lane;
+    bool alive = false;
+    if (r < rend) { const Hdr* h = s.hdr + r; alive = !(h->n_active == 0u && h->a_next == kNever); }
+    const uint32_t m = __ballot_sync(0xffffffffu, alive);
+    uint32_t off = 0;
+    if (lane == 0 && m) off = atomicAdd(cnt, (uint32_t)__popc(m));
+    off = __shfl_sync(0xffffffffu, off, 0);
+    if (alive) out[off + __popc(m & ((1u << lane) - 1u))] = r;
+  }
+}
+void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, uint32_t* out, uint32_t* cnt, cudaStream_t st) {
+  cudaMemsetAsync(cnt, 0, sizeof(uint32_t), st);
+  k_compact_live<<<148, 256, 0, st>>>(s, rbeg, rend, out, cnt);
+}
+
 // ------------------------------------------------------------------ t_last flush (ub_per_request)
 // A request that emitted in the last executed iteration carries its t_last implicitly (== replica clock).
 __global__ void k_flush_tlast(SimDev s) {

@@ -105,6 +105,7 @@ struct StepArgs {
   uint32_t nstat, dynbase;      // k_stream work distribution (set by launch_stream): static replicas per warp, first ticket
   uint32_t rbeg, rend;          // replicas [rbeg, rend) belong to this launch (a round may be split over two streams)
   uint32_t thrS, thrM;          // window size up to which a replica is queued for the S / M kernel
+  const uint32_t* live;         // k_stream, list mode: the replicas to visit are live[rbeg .. rend) (else the indices themselves)
 };
 
 __device__ __forceinline__ void push_list(const StepArgs& A, uint32_t slot, uint32_t r) {

@@ -706,6 +706,7 @@ int step_configure(uint32_t) {
 static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg,
                       uint32_t rend) {
   A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend; A.nstat = A.dynbase = A.tick = 0;
+  A.live = nullptr;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
@@ -713,10 +714,11 @@ static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* co
 }
 
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 uint32_t tick, cudaStream_t st) {
+                 uint32_t tick, const uint32_t* live, uint32_t nlive, cudaStream_t st) {
   StepArgs A;
   make_args(A, s, list, count, iters, rbeg, rend);
   A.tick = tick & 1u;
+  if (live) { A.live = live; A.rbeg = 0; A.rend = nlive; }      // list mode: positions [0, nlive) of the live list
   launch_stream(A, st);
 }
 

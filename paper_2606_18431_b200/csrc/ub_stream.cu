@@ -79,7 +79,8 @@ __device__ __forceinline__ void score(const Rec0& q0, const Rec1& q1, uint32_t k
 // MULTI: several iterations per launch (the resident-state mode: the window is re-read from L2 between them); the
 // one-iteration instance carries none of that either -- the instruction cache (32 KB per SM) is what this kernel
 // competes for, so every instance holds only the code it runs.
-template <bool ADA, bool MULTI>
+// LIST: the replicas to visit come from a compacted list of the unfinished ones (the tail of a run).
+template <bool ADA, bool MULTI, bool LIST>
 __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   __shared__ WarpBuf wbuf[kSWarps];
   const SimDev& s = A.s;
@@ -92,7 +93,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 
   // header, parameters, dirty list and the first two chunks of replica rr -> stage `par` (one cp.async group)
   auto prefetch_replica = [&](const uint32_t rr, const uint32_t par) {
-    if (rr < A.rend) {
+    if (rr != 0xFFFFFFFFu) {
       if (lane < 16) cp16(&X.hdr[par][lane], reinterpret_cast<const uint4*>(s.hdr + rr) + lane);
       const uint4* e0 = reinterpret_cast<const uint4*>(s.E0 + (size_t)rr * Q) + lane;
       const uint4* e1 = reinterpret_cast<const uint4*>(s.E1 + (size_t)rr * Q) + lane;
@@ -108,24 +109,26 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 #define UB_GW (A.rbeg + blockIdx.x * kSWarps + (threadIdx.x >> 5))
   // r: the replica being advanced (its header and first chunks sit in stage `parity`), rn: the one being fetched; the
   // first round of the loop only fetches (one prefetch site: code size)
+  // (ri / rni: their positions in [rbeg, rend) -- the replica numbers themselves unless LIST)
   constexpr uint32_t kNone = 0xFFFFFFFFu;
-  uint32_t r = kNone, rn = UB_GW;
+  uint32_t r = kNone, ri = kNone, rn = kNone, rni = UB_GW;
   uint32_t taken = 1, ticket = 0;
   uint32_t parity = 1;
   // (the ticket counter of the NEXT launch is zeroed here: launches of one part alternate between the two)
   if (blockIdx.x == 0 && threadIdx.x == 0) A.count[4 + 2 * (A.tick ^ 1u)] = 0u;
-  for (;; r = rn, rn = (taken < A.nstat ? UB_GW + taken * nwarps : __shfl_sync(kFull, ticket, 0) + A.dynbase), taken++,
+  for (;; r = rn, ri = rni, rni = (taken < A.nstat ? UB_GW + taken * nwarps : __shfl_sync(kFull, ticket, 0) + A.dynbase), taken++,
           parity ^= 1u) {
     cp_wait<0>();
     __syncwarp();
+    rn = rni < A.rend ? (LIST ? __ldg(A.live + rni) : rni) : kNone;
     prefetch_replica(rn, parity ^ 1u);
     // (inline PTX: the compiler's own atomicAdd broadcasts the result with a shuffle at once, which waits ~600 cycles
     // for the atomic's round trip -- 10 % of all warp time; here the ticket is first read one replica later)
     if (taken >= A.nstat && lane == 0)
       asm volatile("{ .reg .u64 a; .reg .u32 z; mov.u32 z, %%laneid; cvt.u64.u32 a, z; add.u64 a, a, %1; atom.global.add.u32 %0, [a], 1; }"
                    : "=r"(ticket) : "l"(A.count + 4 + 2 * A.tick) : "memory");       // (lane 0: a = the counter)
-    if (r == kNone) continue;
-    if (r >= A.rend) break;
+    if (ri == kNone) continue;
+    if (ri >= A.rend) break;
     const unsigned long long* sh = reinterpret_cast<const unsigned long long*>(X.hdr[parity]);
     // (addresses and per-replica scalars that are needed rarely are re-derived where they are used instead of
     // living in registers across the chunk loop)
@@ -805,12 +808,12 @@ void launch_debug_keys_stream(const SimDev& s, uint32_t r, uint32_t n, uint32_t*
 }
 
 // persistent grid: every warp takes replicas until none is left
-template <bool ADA, bool MULTI> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
+template <bool ADA, bool MULTI, bool LIST> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
   StepArgs A = A0;
   static int ctas_per_sm = 0;
   if (!ctas_per_sm) {
-    cudaFuncSetAttribute(k_stream<ADA, MULTI>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream<ADA, MULTI>, 32 * kSWarps, 0) != cudaSuccess ||
+    cudaFuncSetAttribute(k_stream<ADA, MULTI, LIST>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream<ADA, MULTI, LIST>, 32 * kSWarps, 0) != cudaSuccess ||
         ctas_per_sm < 1)
       ctas_per_sm = 4;
   }
@@ -825,12 +828,14 @@ template <bool ADA, bool MULTI> static void launch_stream_t(const StepArgs& A0, 
   const uint32_t nwarps = grid * kSWarps, share = ((A.rend - A.rbeg) / nwarps) * 7u / 8u;
   A.nstat = share > 2u ? share : 2u;
   A.dynbase = A.rbeg + A.nstat * nwarps;
-  k_stream<ADA, MULTI><<<grid, 32 * kSWarps, 0, st>>>(A);
+  k_stream<ADA, MULTI, LIST><<<grid, 32 * kSWarps, 0, st>>>(A);
 }
 void launch_stream(const StepArgs& A, cudaStream_t st) {
-  if (A.s.ada_ring) launch_stream_t<true, false>(A, st);          // (gamma-Ada: one iteration per launch, ub_api.cu)
-  else if (A.iters > 1u) launch_stream_t<false, true>(A, st);
-  else launch_stream_t<false, false>(A, st);
+  if (A.rend <= A.rbeg) return;
+  if (A.s.ada_ring) launch_stream_t<true, false, false>(A, st);   // (gamma-Ada: one iteration per launch, no list: ub_api.cu)
+  else if (A.iters > 1u) { if (A.live) launch_stream_t<false, true, true>(A, st); else launch_stream_t<false, true, false>(A, st); }
+  else if (A.live) launch_stream_t<false, false, true>(A, st);
+  else launch_stream_t<false, false, false>(A, st);
 }
 
 }  // namespace ub

@@ -28,3 +28,15 @@ def aggregate(request_steps_timed: float, request_steps_all: float, ms: float, t
         m_ = tot.clone(); dist.all_reduce(m_, dist.ReduceOp.MAX)
         return s_[0].item(), s_[1].item(), m_[2].item(), m_[3].item()
     return tot[0].item(), tot[1].item(), tot[2].item(), tot[3].item()
+
+
+def gather_replica_stats(table, device, world: int):
+    """The one exchange of the job: every rank's [R_rank][W] per-replica statistics, concatenated
+    in rank order (= replica order of the unsharded job) on every rank.  `table`: int64 numpy array; returns numpy."""
+    import numpy as np
+    t = torch.as_tensor(np.ascontiguousarray(table, dtype=np.int64), device=device)
+    if world == 1:
+        return t.cpu().numpy()
+    out = [torch.empty_like(t) for _ in range(world)]
+    dist.all_gather(out, t)
+    return torch.cat(out, 0).cpu().numpy()
