@@ -27,6 +27,8 @@ struct ub_sim {
   uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([5] = finished replicas)
   uint32_t* d_live; uint32_t* d_livecnt; // ub_run's tail: the unfinished replicas of each part of a round, compacted
   bool use_list; uint32_t livecnt[ub::kMaxSplit];
+  uint32_t* d_drift; uint32_t* d_drift_live; uint32_t ndrift, drift_livecnt;   // the drift group (SRPT / LAS replicas): launched
+                                                                            // beside the parts, from its own list (ub_stream.cu)
   int64_t* d_ada_ring; AdaState* d_ada_state; int64_t* d_ada_grid;   // gamma-Ada (M13), null when off
   std::vector<int64_t> h_ada_grid;
   uint2* d_evbuf;                        // per-iteration event scratch [R][min(M,Q)]
@@ -89,20 +91,21 @@ int ub_create(const ub_config* c, ub_sim** out) {
   s->have_trace = s->have_reps = false;
   s->d_TR = nullptr; s->d_lut = nullptr;
   s->last_ms = 0.f; s->last_launches = 0;
-  s->use_list = false;
-  s->nsplit = c->n_replicas >= 8192 ? 2 : 1;          // (measured on config 5: 2 parts 5.9e10, 4 parts 5.5e10 request-steps/s)
+  s->use_list = false; s->ndrift = 0; s->drift_livecnt = 0;
+  s->nsplit = c->n_replicas >= 8192 ? 2 : 1;          // (at most kMaxSplit - 1: the last set of lists is the drift group's)          // (measured on config 5: 2 parts 5.9e10, 4 parts 5.5e10 request-steps/s)
   const size_t R = c->n_replicas, Q = c->queue_cap, N = c->max_requests, NT = c->n_traces;
   int rc = UB_OK;
   if ((rc = dmalloc(&s->d_E0, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_E1, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_hdr, R)) ||
       (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
       (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
-      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_live, R)) || (rc = dmalloc(&s->d_livecnt, kMaxSplit)) || (rc = dmalloc(&s->d_list, 4 * kMaxSplit * R)) || (rc = dmalloc(&s->d_count, 8 * kMaxSplit)) ||
+      (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_live, R)) || (rc = dmalloc(&s->d_livecnt, kMaxSplit + 1)) ||
+      (rc = dmalloc(&s->d_drift, R)) || (rc = dmalloc(&s->d_drift_live, R)) || (rc = dmalloc(&s->d_list, 4 * kMaxSplit * R)) || (rc = dmalloc(&s->d_count, 8 * kMaxSplit)) ||
       (rc = dmalloc(&s->d_evbuf, R * (size_t)(c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap)))) {
     ub_destroy(s);
     return rc;
   }
-  if (cudaMallocHost((void**)&s->h_word, (2 + kMaxSplit) * sizeof(unsigned long long)) != cudaSuccess ||
+  if (cudaMallocHost((void**)&s->h_word, (3 + kMaxSplit) * sizeof(unsigned long long)) != cudaSuccess ||
       cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess ||
       cudaStreamCreateWithFlags(&s->aux[0], cudaStreamNonBlocking) != cudaSuccess ||
       cudaStreamCreateWithFlags(&s->aux[1], cudaStreamNonBlocking) != cudaSuccess ||
@@ -138,7 +141,7 @@ void ub_destroy(ub_sim* s) {
   cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_TR);
   cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
-  cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_evbuf); cudaFree(s->d_live); cudaFree(s->d_livecnt);
+  cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_evbuf); cudaFree(s->d_live); cudaFree(s->d_livecnt); cudaFree(s->d_drift); cudaFree(s->d_drift_live);
   cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);
   if (s->h_word) cudaFreeHost(s->h_word);
   if (s->ev0) cudaEventDestroy(s->ev0);
@@ -286,8 +289,19 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   {
     bool all = s->dev.blk_shift < 32u;
     for (size_t r = 0; r < R && all; r++)
-      all = (reps[r].policy == UB_FCFS || reps[r].policy == UB_BOOST) && reps[r].signal_mode == 0 && reps[r].quant_mode == 0;
+      all = reps[r].policy != UB_DISTBOOST && reps[r].signal_mode == 0 && reps[r].quant_mode == 0;
     s->dev.all_stream = all ? 1u : 0u;
+  }
+  {
+    // the drift group: replicas whose keys move with every token (SRPT, LAS) and that the streaming kernel covers
+    std::vector<uint32_t> dl;
+    if (s->dev.blk_shift < 32u)
+      for (size_t r = 0; r < R; r++)
+        if ((reps[r].policy == UB_SRPT || reps[r].policy == UB_LAS) && reps[r].signal_mode == 0 && reps[r].quant_mode == 0)
+          dl.push_back((uint32_t)r);
+    s->ndrift = (uint32_t)dl.size();
+    if (!dl.empty()) CK(cudaMemcpyAsync(s->d_drift, dl.data(), dl.size() * 4, cudaMemcpyHostToDevice, s->stream));
+    CK(cudaStreamSynchronize(s->stream));                             // (dl is a local)
   }
   cudaFree(s->d_lut); s->d_lut = nullptr;
   int rc = dmalloc(&s->d_lut, s->h_lut.size()); if (rc) return rc;
@@ -317,33 +331,47 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
   const uint32_t ipl = (!ada && s->cfg.iters_per_launch > 1) ? s->cfg.iters_per_launch : 1;
   const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
   const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
+  // the drift group (SRPT / LAS replicas) is one more independent set of replicas: its launches go to a stream of their
+  // own beside the parts, with the last set of work lists and counters
+  constexpr uint32_t DP = kMaxSplit - 1;
+  const bool lst = s->use_list && !ada;
+  const uint32_t nd = ada ? 0u : (lst ? s->drift_livecnt : s->ndrift);
+  const uint32_t* dlist = lst ? s->d_drift_live : s->d_drift;
+  cudaStream_t dst = s->aux[2];
   uint32_t nl = 0;
-  if (ns > 1) {
+  if (ns > 1 || nd) {
     CK(cudaEventRecord(s->ev_fork, s->stream));
     for (uint32_t i = 1; i < ns; i++) CK(cudaStreamWaitEvent(s->aux[i - 1], s->ev_fork, 0));
+    if (nd) CK(cudaStreamWaitEvent(dst, s->ev_fork, 0));
   }
   while (n_iters > 0) {
     const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
     for (uint32_t i = 0; i < ns; i++) {
       const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
       if (ada) launch_gamma_ada(s->dev, rb, re, i ? s->aux[i - 1] : s->stream);
-      const bool lst = s->use_list && !ada;
       launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, s->round_no,
-                  lst ? s->d_live + rb : nullptr, lst ? s->livecnt[i] : 0u, i ? s->aux[i - 1] : s->stream);
+                  lst ? s->d_live + rb : nullptr, lst ? s->livecnt[i] : 0u, false, i ? s->aux[i - 1] : s->stream);
     }
+    if (nd) launch_step(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, k, 0, nd, s->round_no, dlist, nd, true, dst);
     n_iters -= k; nl++; s->round_no++;
     // what k_stream queued for the team kernels runs at the end of the call (all owed iterations at once); with
     // gamma-Ada after every round, because UPDATEGAMMA sits between the iterations
-    if (ada || n_iters == 0)
+    if (ada || n_iters == 0) {
       for (uint32_t i = 0; i < ns; i++) {
         const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
         flush_slow(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, rb, re, i ? s->aux[i - 1] : s->stream);
       }
+      if (nd) flush_slow(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, 0, nd, dst);
+    }
   }
-  if (ns > 1) {
+  if (ns > 1 || nd) {
     for (uint32_t i = 1; i < ns; i++) {
       CK(cudaEventRecord(s->ev_join[i - 1], s->aux[i - 1]));
       CK(cudaStreamWaitEvent(s->stream, s->ev_join[i - 1], 0));
+    }
+    if (nd) {
+      CK(cudaEventRecord(s->ev_join[2], dst));
+      CK(cudaStreamWaitEvent(s->stream, s->ev_join[2], 0));
     }
   }
   *launches = nl;
@@ -381,14 +409,16 @@ static int compact_live(ub_sim* s, uint64_t* live) {
   const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
   for (uint32_t i = 0; i < ns; i++) {
     const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
-    launch_compact_live(s->dev, rb, re, s->d_live + rb, s->d_livecnt + i, s->stream);
+    launch_compact_live(s->dev, rb, re, nullptr, false, s->d_live + rb, s->d_livecnt + i, s->stream);
   }
+  launch_compact_live(s->dev, 0, s->ndrift, s->d_drift, true, s->d_drift_live, s->d_livecnt + ns, s->stream);
   uint32_t* hc = reinterpret_cast<uint32_t*>(s->h_word + 2);
-  CK(cudaMemcpyAsync(hc, s->d_livecnt, ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaMemcpyAsync(hc, s->d_livecnt, (ns + 1) * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
   CK(cudaGetLastError());
   uint64_t tot = 0;
   for (uint32_t i = 0; i < ns; i++) { s->livecnt[i] = hc[i]; tot += hc[i]; }
+  s->drift_livecnt = hc[ns]; tot += hc[ns];
   s->use_list = true;
   *live = tot;
   return UB_OK;
@@ -736,7 +766,7 @@ static int debug_keys_impl(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* 
   if (!s->have_reps) return UB_ESTATE;
   if (stream_scorer) {                             // the streaming kernel covers FCFS / BOOST with the paper's signal and quantiser
     const ub_replica& q = s->h_reps[r];
-    if (!(q.policy == UB_FCFS || q.policy == UB_BOOST) || q.signal_mode != UB_SIG_UNIFIED || q.quant_mode != UB_Q_GEOMETRIC)
+    if (q.policy == UB_DISTBOOST || q.signal_mode != UB_SIG_UNIFIED || q.quant_mode != UB_Q_GEOMETRIC || s->dev.blk_shift >= 32u)
       return UB_EINVAL;
   }
   if (set_dev(s)) return UB_ECUDA;

@@ -126,14 +126,25 @@ void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* li
   k_count_live<<<1, 1, 0, st>>>(count, R, live);
 }
 
-// The unfinished replicas of [rbeg, rend), compacted (ub_run's tail: the streaming kernel then visits only these).
-// A replica is finished when its trace is exhausted and nothing is active (M6); finished replicas never come back.
-__global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, uint32_t* out, uint32_t* cnt) {
+// The unfinished replicas among positions [rbeg, rend) -- of the list `in`, else the replica numbers themselves --
+// that belong to the drift group (SRPT / LAS) or to the main one, compacted (ub_run's tail: the streaming kernel then
+// visits only these).  A replica is finished when its trace is exhausted and nothing is active (M6); finished
+// replicas never come back.
+__global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, const uint32_t* in, uint32_t drift_group, uint32_t* out,
+                               uint32_t* cnt) {
   const uint32_t lane = threadIdx.x & 31u;
   for (uint32_t base = rbeg + (blockIdx.x * blockDim.x + threadIdx.x - lane); base < rend; base += gridDim.x * blockDim.x) {
-    const uint32_t r = base + lane;
+    const uint32_t i = base + lane;
     bool alive = false;
-    if (r < rend) { const Hdr* h = s.hdr + r; alive = !(h->n_active == 0u && h->a_next == kNever); }
+    uint32_t r = 0;
+    if (i < rend) {
+      r = in ? in[i] : i;
+      const Hdr* h = s.hdr + r;
+      const RepPar& q = h->par;
+      const uint32_t dg = (!s.ada_ring && (q.policy == 1u || q.policy == 3u) && q.signal_mode == 0u && q.quant_mode == 0u &&
+                           s.blk_shift < 32u) ? 1u : 0u;
+      alive = !(h->n_active == 0u && h->a_next == kNever) && dg == drift_group;
+    }
     const uint32_t m = __ballot_sync(0xffffffffu, alive);
     uint32_t off = 0;
     if (lane == 0 && m) off = atomicAdd(cnt, (uint32_t)__popc(m));
@@ -141,9 +152,10 @@ __global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, uint32_t*
     if (alive) out[off + __popc(m & ((1u << lane) - 1u))] = r;
   }
 }
-void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, uint32_t* out, uint32_t* cnt, cudaStream_t st) {
+void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, const uint32_t* in, bool drift_group, uint32_t* out,
+                         uint32_t* cnt, cudaStream_t st) {
   cudaMemsetAsync(cnt, 0, sizeof(uint32_t), st);
-  k_compact_live<<<148, 256, 0, st>>>(s, rbeg, rend, out, cnt);
+  if (rend > rbeg) k_compact_live<<<148, 256, 0, st>>>(s, rbeg, rend, in, drift_group ? 1u : 0u, out, cnt);
 }
 
 // ------------------------------------------------------------------ t_last flush (ub_per_request)

@@ -96,7 +96,7 @@ struct SimDev {                 // kernel argument (by value)
 
 // kernels (ub_step.cu, ub_aux.cu)
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 uint32_t tick, const uint32_t* live, uint32_t nlive, cudaStream_t st);
+                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, cudaStream_t st);
 void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, cudaStream_t st);
 void launch_stream(const struct StepArgs& A, cudaStream_t st);    // ub_stream.cu
 void launch_debug_keys_stream(const SimDev& s, uint32_t r, uint32_t n, uint32_t* id, unsigned long long* okey, cudaStream_t st);
@@ -107,7 +107,8 @@ void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, 
                           uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st);
 void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st);
 void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* live, cudaStream_t st);
-void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, uint32_t* out, uint32_t* cnt, cudaStream_t st);
+void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, const uint32_t* in, bool drift_group, uint32_t* out,
+                         uint32_t* cnt, cudaStream_t st);
 void launch_flush_tlast(const SimDev& s, cudaStream_t st);
 struct StatsDev {               // device-side result of the percentile reduction, one per replica
   int64_t ttft[3], ttlt[3], tbt[3];

@@ -40,6 +40,7 @@ struct TeamScratch {            // per team, in shared memory
   unsigned long long acc64[6];  // rare-event accumulators
   uint32_t acc32[4];
   uint32_t ndirty;             // next iteration's dirty-list length
+  unsigned long long smax[2][8]; // exchange buffer of the prefix maximum
 };
 
 template <int WARPS> struct Team {
@@ -66,6 +67,30 @@ template <int WARPS> struct Team {
       for (int i = 0; i < WARPS; i++) { uint32_t x = buf[i]; if (i < warp) off += x; tot += x; }
       total = tot;
       return w + off;
+    }
+  }
+  // exclusive prefix maximum over the team in thread order (0 in front of the first thread), and the team maximum
+  __device__ __forceinline__ uint64_t scanmax_excl(uint64_t v, uint64_t& total) {
+    uint64_t w = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint64_t t = __shfl_up_sync(0xffffffffu, w, o);
+      if (lane >= o && t > w) w = t;
+    }
+    uint64_t ex = __shfl_up_sync(0xffffffffu, w, 1);
+    if (lane == 0) ex = 0ull;
+    if constexpr (WARPS == 1) {
+      total = __shfl_sync(0xffffffffu, w, 31);
+      return ex;
+    } else {
+      unsigned long long* buf = ts->smax[phase & 1]; phase++;
+      if (lane == 31) buf[warp] = w;
+      __syncthreads();
+      uint64_t off = 0, tot = 0;
+#pragma unroll
+      for (int i = 0; i < WARPS; i++) { const uint64_t x = buf[i]; if (i < warp && x > off) off = x; if (x > tot) tot = x; }
+      total = tot;
+      return ex > off ? ex : off;
     }
   }
   __device__ __forceinline__ bool any(bool p) const {
@@ -588,6 +613,34 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
       }
     }
 
+    // SRPT / LAS keys drift with every emitted token.  The streaming kernel trusts the dirty hints, so they must cover
+    // the drift too: a request whose next (class, key, id) sorts in front of one that is written before it is hinted
+    // (the same rule as in ub_stream.cu process()).
+    if (par.policy == 1 || par.policy == 3) {
+      uint64_t carry = 0;
+#pragma unroll
+      for (int c = 0; c < E; c++) {
+        const uint32_t base = c * TH;
+        if (base < n) {
+          const uint32_t pos = base + tid;
+          const bool keep = pos < n && !gone[c];
+          uint64_t comp = 0;
+          if (keep) {
+            const uint32_t f = r1[c].flags;
+            const uint32_t bin2 = bin_of(par, s.k, signal_of(par, r0[c].P, r0[c].D, r1[c].d));
+            const uint32_t klass2 = (par.guard && (f & F_RESIDENT) && (f >> F_LOCK_SHIFT) == bin2 + 1u) ? 0u : 1u;
+            const uint32_t key2 = par.policy == 1 ? r0[c].D - r1[c].d : signal_of(par, r0[c].P, r0[c].D, r1[c].d);
+            comp = ((uint64_t)klass2 << 63) | ((uint64_t)key2 << 32) | (uint64_t)r1[c].id;
+          }
+          uint64_t tot;
+          uint64_t before = tm.scanmax_excl(comp, tot);
+          if (carry > before) before = carry;
+          if (keep && comp < before) r1[c].flags |= F_DIRTY;
+          if (tot > carry) carry = tot;
+        }
+      }
+    }
+
     // ---------------- write back in priority order, dropping completed requests
     uint32_t n_new = 0;
 #pragma unroll
@@ -706,7 +759,7 @@ int step_configure(uint32_t) {
 static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg,
                       uint32_t rend) {
   A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend; A.nstat = A.dynbase = A.tick = 0;
-  A.live = nullptr;
+  A.live = nullptr; A.drift = 0;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
@@ -714,11 +767,12 @@ static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* co
 }
 
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 uint32_t tick, const uint32_t* live, uint32_t nlive, cudaStream_t st) {
+                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, cudaStream_t st) {
   StepArgs A;
   make_args(A, s, list, count, iters, rbeg, rend);
   A.tick = tick & 1u;
-  if (live) { A.live = live; A.rbeg = 0; A.rend = nlive; }      // list mode: positions [0, nlive) of the live list
+  A.drift = drift ? 1u : 0u;
+  if (live) { A.live = live; A.rbeg = 0; A.rend = nlive; }      // list mode: positions [0, nlive) of the list
   launch_stream(A, st);
 }
 

@@ -59,9 +59,11 @@ struct __align__(16) WarpBuf {             // per warp, 10 KB
 static_assert(sizeof(Hdr) == 256, "cp.async copies the header as sixteen 16-byte pieces");
 
 // a1 (M3-M5): sig = P + d; bin = Eq. 8 exponent; pi = a - b_gamma(w_hat) - delta if
-// resident (Eq. 7); key = class<<63 | (pi + 2^62); class 0 = MemGuard-locked resident.  All 32 lanes must call it.
+// resident (Eq. 7); key = class<<63 | (pi + 2^62); class 0 = MemGuard-locked resident.  The baselines keyed by a size
+// replace pi: SRPT D - d, LAS sig, SJF D, SPF P (the caller passes lutv = 0 and delta = 0 for
+// them).  policy is warp-uniform.  All 32 lanes must call it.
 __device__ __forceinline__ void score(const Rec0& q0, const Rec1& q1, uint32_t k, int64_t lutv, int64_t delta,
-                                      bool guard, uint64_t& key, uint32_t& bin) {
+                                      bool guard, uint32_t policy, uint64_t& key, uint32_t& bin) {
   const uint32_t sig = q0.P + q1.d;
   const uint32_t sg = sig > k ? sig : k;
   uint32_t b = (uint32_t)(__clz(k) - __clz(sg));
@@ -69,18 +71,44 @@ __device__ __forceinline__ void score(const Rec0& q0, const Rec1& q1, uint32_t k
   const uint32_t lo = __shfl_sync(kFull, (uint32_t)lutv, (int)b);
   const uint32_t hi = __shfl_sync(kFull, (uint32_t)((uint64_t)lutv >> 32), (int)b);
   const bool res = (q1.flags & F_RESIDENT) != 0;
-  const int64_t kv = q0.a - (int64_t)(((uint64_t)hi << 32) | lo) - (res ? delta : 0ll);
+  int64_t base = q0.a;
+  if (policy != 0u && policy != 2u)
+    base = (int64_t)(policy == 1u ? q0.D - q1.d : (policy == 3u ? sig : (policy == 4u ? q0.D : q0.P)));
+  const int64_t kv = base - (int64_t)(((uint64_t)hi << 32) | lo) - (res ? delta : 0ll);
   const bool locked = guard && res && (q1.flags >> F_LOCK_SHIFT) == b + 1u;
   key = (uint64_t)(kv + kKeyBias) | (locked ? 0ull : (1ull << 63));
   bin = b;
+}
+
+// The re-key rule of the drifting keys (SRPT, LAS), kept out of line: the streaming kernel competes for the instruction
+// cache and the arrival-keyed policies never come here.  comp = the request's next (class, key, id), 0 for a lane
+// whose request leaves; kmax = the largest one written so far (updated).  True when the lane's request sorts in
+// front of one written before it.
+__device__ __noinline__ bool drift_out_of_order(const uint64_t comp, uint64_t& kmax) {
+  const int lane = threadIdx.x & 31;
+  uint64_t pm = comp;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint64_t t = __shfl_up_sync(kFull, pm, o);
+    if (lane >= o && t > pm) pm = t;
+  }
+  uint64_t before = __shfl_up_sync(kFull, pm, 1);
+  if (lane == 0) before = 0ull;
+  if (kmax > before) before = kmax;
+  const uint64_t top = __shfl_sync(kFull, pm, 31);
+  if (top > kmax) kmax = top;
+  return comp != 0ull && comp < before;
 }
 
 // ADA: the gamma-Ada instance (per-level boost tables, latency window); the static instance carries none of it.
 // MULTI: several iterations per launch (the resident-state mode: the window is re-read from L2 between them); the
 // one-iteration instance carries none of that either -- the instruction cache (32 KB per SM) is what this kernel
 // competes for, so every instance holds only the code it runs.
-// LIST: the replicas to visit come from a compacted list of the unfinished ones (the tail of a run).
-template <bool ADA, bool MULTI, bool LIST>
+// LIST: the replicas to visit come from a list (the unfinished ones in the tail of a run; the drift group).
+// DRIFT: the replicas whose keys drift with every token (SRPT, LAS) are advanced by an instance of their own, launched
+// over their list beside the main one: the extra re-key rule and its state stay out of the main instance, whose
+// register budget and instruction-cache footprint decide the headline number.
+template <bool ADA, bool MULTI, bool LIST, bool DRIFT>
 __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
   __shared__ WarpBuf wbuf[kSWarps];
   const SimDev& s = A.s;
@@ -134,7 +162,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     // living in registers across the chunk loop)
 #define UB_H64 (reinterpret_cast<unsigned long long*>(s.hdr + r))
 #define UB_TR (s.TR + (size_t)reinterpret_cast<const Hdr*>(X.hdr[parity])->par.trace_id * s.N)
-#define UB_DELTA (reinterpret_cast<const Hdr*>(X.hdr[parity])->par.delta)
+#define UB_DELTA (hyst ? reinterpret_cast<const Hdr*>(X.hdr[parity])->par.delta : 0ll)
     uint32_t n = (uint32_t)sh[13];
     if (n == 0 && (int64_t)sh[2] == kNever) continue;                 // finished its trace
     {
@@ -153,8 +181,19 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
     const bool isboost = par.policy == 2;
     const bool guard = par.guard != 0;
 
-    // the streaming path covers the arrival-keyed policies with the paper's signal and quantiser
-    bool slow = !(par.policy == 0 || par.policy == 2) || par.signal_mode != 0 || par.quant_mode != 0 || blk_sh >= 32u;
+    // the streaming path covers the paper's signal and quantiser under every policy but DistBoost (whose decode-queue
+    // key is the request's first-token time, a gather from the per-request outputs)
+    bool slow = par.policy > 5 || par.signal_mode != 0 || par.quant_mode != 0 || blk_sh >= 32u;
+    const bool hyst = par.policy == 0 || par.policy == 2;             // Eq. 7 applies to the arrival-keyed policies
+    // SRPT / LAS keys drift: every emitted token moves the request's key by one.  The order is then kept by one more
+    // re-key rule (in process()): a request whose next key sorts in front of one written before it is listed dirty.
+    constexpr bool drift = DRIFT;
+    if constexpr (!DRIFT) {
+      if (!slow && (par.policy == 1 || par.policy == 3)) {   // (a member of the drift group: ub_set_replicas has the same test)
+        if constexpr (ADA) slow = true;        // (the gamma-Ada instance has no drift twin: the team kernels take them)
+        else continue;                         // the drift instance's launch advances this replica
+      }
+    }
     // boost table in registers: lane b holds LUT[b] (Eq. 2 in fixed point, built on the host, M4); FCFS: all 0
     int64_t lutv = 0;
     // (a gamma-Ada replica owns one table per grid level, Hdr::level selects; 0 for a static replica)
@@ -244,7 +283,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const Rec0 q0 = *reinterpret_cast<const Rec0*>(&v0);
         const Rec1 q1 = *reinterpret_cast<const Rec1*>(&v1);
         uint64_t sk; uint32_t sb;
-        score(q0, q1, k, lutv, UB_DELTA, guard, sk, sb);
+        score(q0, q1, k, lutv, UB_DELTA, guard, par.policy, sk, sb);
         uint32_t rank = 0;
         if (m > 1u) {
 #pragma unroll 1
@@ -274,6 +313,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       // (each field < 2^16: M, Q <= 2048, T <= 65535); swap-ins (rare) are summed in shared memory
       uint32_t de = 0, ps = 0, kres = 0, evl = 0, evu = 0;
       uint32_t rhi = 0;                                               // 1 + the last new position this lane gave to a resident
+      uint64_t kmax = 0;                                              // drift: the largest next (class, key, id) written so far
       uint32_t outpos = 0, nev = 0, ndnew = 0, n_done = 0;
       uint32_t dptr = 0;                                              // next parked request to merge
 
@@ -380,7 +420,15 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const bool res2 = (nf & F_RESIDENT) != 0;
         const uint32_t klass = (uint32_t)(key >> 63);
         const uint32_t klass2 = (guard && res2 && b2 == bin) ? 0u : 1u;
-        const bool dirty = (((nf ^ of) & F_RESIDENT) != 0) || (isboost && b2 != bin) || (klass2 != klass);
+        bool dirty = (((nf ^ of) & F_RESIDENT) != 0) || (isboost && b2 != bin) || (klass2 != klass);
+        if constexpr (DRIFT) {
+          // next iteration's (class, key, id) of every request that stays, in the order written: whoever sorts in
+          // front of a request written before it must be re-merged (the others then still form a sorted stream)
+          const uint32_t key2 = par.policy == 1 ? w0.D - d2 : sig + (emitted ? 1u : 0u);
+          const bool stays = valid && !gone;
+          const uint64_t comp = stays ? (((uint64_t)klass2 << 63) | ((uint64_t)key2 << 32) | (uint64_t)w1.id) : 0ull;
+          if (drift_out_of_order(comp, kmax)) dirty = true;
+        }
         if (res2) nf |= (bin + 1u) << F_LOCK_SHIFT;
         if (klass) nf |= F_KLASS1;
         if (dirty) nf |= F_DIRTY;
@@ -443,7 +491,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         // ---------------- (A) chunks of MemGuard-locked residents in steady decode (each wants one token, emits it,
         // neither completes nor crosses its Eq. 8 threshold) that fit as a whole: class 0 in stored order (so in front
         // of a parked request of class 1), nothing is re-keyed, every record advances by one token (M2, M7, M10)
-        if (mode == 0u && guard && c < nch) {
+        if (mode == 0u && guard && !drift && c < nch) {
           const bool pend = dptr < m;
           if (!pend || (X.skb[dptr].y >> 31)) {
             do {
@@ -504,7 +552,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         }
         // ---------------- (T) behind the walk, nothing parked left: chunks of waiting requests (not resident, nothing
         // to finalise) only move up when requests in front of them completed
-        if (mode != 0u && dptr >= m && c >= dlo + dspan) {
+        if (mode != 0u && dptr >= m && !drift && c >= dlo + dspan) {
           while (c < nch) {
             wait_chunk(c, outpos > c * 32u);
             const uint4* st = stage_of(c);
@@ -534,8 +582,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         const Rec1 r1 = *reinterpret_cast<const Rec1*>(&c1);
         const uint32_t cv = valid_of(c);
         uint64_t key; uint32_t bin;
-        score(r0, r1, k, lutv, UB_DELTA, guard, key, bin);
-        if (mode != 0u && cv != 0u) {
+        score(r0, r1, k, lutv, UB_DELTA, guard, par.policy, key, bin);
+        if (mode != 0u && cv != 0u && !drift) {
           // ---- behind the walk: a chunk of waiting requests (not resident, nothing to finalise) that sorts in front
           // of the next parked request, if any, only moves up
           const bool steady = (r1.flags & ~F_SWAPPED) == F_KLASS1;
@@ -799,7 +847,7 @@ __global__ void k_debug_keys_stream(const SimDev s, const uint32_t r, const uint
     q0.a = 0; q0.P = 1; q0.D = 1; q1.id = 0; q1.d = 0; q1.cached = 0; q1.flags = 0;
     if (p < n) { q0 = s.E0[(size_t)r * s.Q + p]; q1 = s.E1[(size_t)r * s.Q + p]; }
     uint64_t key; uint32_t bin;
-    score(q0, q1, s.k, lutv, par.delta, par.guard != 0, key, bin);
+    score(q0, q1, s.k, lutv, (par.policy == 0 || par.policy == 2) ? par.delta : 0ll, par.guard != 0, par.policy, key, bin);
     if (p < n) { id[p] = q1.id; okey[p] = key; }
   }
 }
@@ -808,12 +856,12 @@ void launch_debug_keys_stream(const SimDev& s, uint32_t r, uint32_t n, uint32_t*
 }
 
 // persistent grid: every warp takes replicas until none is left
-template <bool ADA, bool MULTI, bool LIST> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
+template <bool ADA, bool MULTI, bool LIST, bool DRIFT> static void launch_stream_t(const StepArgs& A0, cudaStream_t st) {
   StepArgs A = A0;
   static int ctas_per_sm = 0;
   if (!ctas_per_sm) {
-    cudaFuncSetAttribute(k_stream<ADA, MULTI, LIST>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream<ADA, MULTI, LIST>, 32 * kSWarps, 0) != cudaSuccess ||
+    cudaFuncSetAttribute(k_stream<ADA, MULTI, LIST, DRIFT>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, k_stream<ADA, MULTI, LIST, DRIFT>, 32 * kSWarps, 0) != cudaSuccess ||
         ctas_per_sm < 1)
       ctas_per_sm = 4;
   }
@@ -828,14 +876,17 @@ template <bool ADA, bool MULTI, bool LIST> static void launch_stream_t(const Ste
   const uint32_t nwarps = grid * kSWarps, share = ((A.rend - A.rbeg) / nwarps) * 7u / 8u;
   A.nstat = share > 2u ? share : 2u;
   A.dynbase = A.rbeg + A.nstat * nwarps;
-  k_stream<ADA, MULTI, LIST><<<grid, 32 * kSWarps, 0, st>>>(A);
+  k_stream<ADA, MULTI, LIST, DRIFT><<<grid, 32 * kSWarps, 0, st>>>(A);
 }
 void launch_stream(const StepArgs& A, cudaStream_t st) {
   if (A.rend <= A.rbeg) return;
-  if (A.s.ada_ring) launch_stream_t<true, false, false>(A, st);   // (gamma-Ada: one iteration per launch, no list: ub_api.cu)
-  else if (A.iters > 1u) { if (A.live) launch_stream_t<false, true, true>(A, st); else launch_stream_t<false, true, false>(A, st); }
-  else if (A.live) launch_stream_t<false, false, true>(A, st);
-  else launch_stream_t<false, false, false>(A, st);
+  if (A.drift) {                                                   // the drift group always comes as a list
+    if (A.iters > 1u) launch_stream_t<false, true, true, true>(A, st); else launch_stream_t<false, false, true, true>(A, st);
+  }
+  else if (A.s.ada_ring) launch_stream_t<true, false, false, false>(A, st);   // (gamma-Ada: one iteration per launch, no list: ub_api.cu)
+  else if (A.iters > 1u) { if (A.live) launch_stream_t<false, true, true, false>(A, st); else launch_stream_t<false, true, false, false>(A, st); }
+  else if (A.live) launch_stream_t<false, false, true, false>(A, st);
+  else launch_stream_t<false, false, false, false>(A, st);
 }
 
 }  // namespace ub
