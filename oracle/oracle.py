@@ -87,6 +87,8 @@ def lib():
         L.orc_tbt_edge.argtypes = [I64]; L.orc_tbt_edge.restype = I64
         L.orc_percentile_curve.argtypes = [C.c_void_p, I64, C.c_void_p, I64, C.c_void_p]
         L.orc_slo_attainment.argtypes = [C.c_void_p, I64, C.c_void_p, I64, C.c_void_p]
+        L.orc_preempt_time.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_class_percentiles.argtypes = [C.c_void_p, I64, I64, I64, C.c_void_p, I64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_set_gamma_ada.argtypes = [C.c_void_p, P(OrcGammaAda), C.c_void_p]
         L.orc_gamma_state.argtypes = [C.c_void_p, I64, P(I64), P(I64), P(I64)]
         L.orc_gamma_grid.argtypes = [C.c_void_p, C.c_void_p]
@@ -173,6 +175,21 @@ class OracleSim:
         out = np.zeros((self.R, len(pm)), np.int64)
         _chk(lib().orc_percentile_curve(self._h, int(which), pm.ctypes.data, len(pm), out.ctypes.data))
         return out
+
+    def preempt_time(self):
+        """[R][N] int64 microseconds each request spent preempted (rule M15)."""
+        out = np.zeros((self.R, self.N), np.int64)
+        _chk(lib().orc_preempt_time(self._h, out.ctypes.data))
+        return out
+
+    def class_percentiles(self, which, len_lo, len_hi, permille):
+        """(percentiles [R][n], count [R], sum [R]) of TTFT (0) / TTLT (1) / preemption time (2) over the completed
+        requests with len_lo <= P + D <= len_hi."""
+        pm = np.ascontiguousarray(permille, np.int64)
+        out = np.zeros((self.R, len(pm)), np.int64); cnt = np.zeros(self.R, np.int64); tot = np.zeros(self.R, np.int64)
+        _chk(lib().orc_class_percentiles(self._h, int(which), int(len_lo), int(len_hi), pm.ctypes.data, len(pm),
+                                         out.ctypes.data, cnt.ctypes.data, tot.ctypes.data))
+        return out, cnt, tot
 
     def slo_attainment(self, which, threshold_us):
         thr = np.ascontiguousarray(threshold_us, np.int64)

@@ -25,6 +25,8 @@ typedef struct {
   int64_t t_first, t_last;
   uint32_t n_evict, n_evict_unforced;
   int32_t completed;
+  int64_t preempt_since;  /* M15: start time of the iteration that evicted it, -1 while it is not preempted */
+  int64_t t_preempt;      /* M15: total time spent preempted so far */
 } orc_req;
 
 typedef struct {
@@ -230,7 +232,7 @@ int orc_set_replicas(orc_sim* s, const orc_replica* reps) {
     x->active = (int32_t*)calloc((size_t)c->queue_cap, sizeof(int32_t));
     x->hist = (uint32_t*)calloc(TBT_BINS, sizeof(uint32_t));
     if (!x->req || !x->active || !x->hist) return ORC_ENOMEM;
-    for (int64_t i = 0; i < n; i++) { x->req[i].t_first = -1; x->req[i].t_last = -1; x->req[i].lockbin = -1; }
+    for (int64_t i = 0; i < n; i++) { x->req[i].t_first = -1; x->req[i].t_last = -1; x->req[i].lockbin = -1; x->req[i].preempt_since = -1; }
     /* boost table (M4): one entry per bin; EXACT quantiser => one entry per signal value */
     int64_t nb = LUT_CAP_GEOM;
     if (x->par.quant_mode == ORC_Q_EXACT) {
@@ -460,6 +462,10 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
       newblocked = 1; continue;
     }
     e[j].want = want; C += foot; tok += want; cnt++;
+    if (q->preempt_since >= 0) {                         /* M15: back on the device -- the preemption ends where this iteration starts */
+      q->t_preempt += x->t - q->preempt_since;
+      q->preempt_since = -1;
+    }
     if (q->d >= 1 && rem == 1) decode_seqs++; else prefill_tokens += want;   /* M9 */
     ev_add(&ev, EV_ADMIT, (uint32_t)e[j].id, (uint32_t)want);
     if (q->swapped) {                                    /* swap-in on admission (M9) */
@@ -494,6 +500,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
       e[j].evict = 1;
     }
     q->resident = 0; q->lockbin = -1; q->n_evict++;
+    q->preempt_since = x->t;                             /* M15: preempted from the start of this iteration on */
     if (e[j].klass == 1) q->n_evict_unforced++;
     sumres -= res;
   }
@@ -717,6 +724,55 @@ int orc_percentile_curve(orc_sim* s, int64_t which, const int64_t* permille, int
       if (rank > m) rank = m;
       out[r * n + k] = v[rank - 1];
     }
+  }
+  free(v);
+  return ORC_OK;
+}
+
+/* M15 / per-class reductions (Tables 3-5): over the completed
+ * requests of a replica whose total length P + D lies in [len_lo, len_hi], the nearest-rank percentiles (t_p of
+ * PAPER.md:225, rank ceil(p m / 1000)) of TTFT (which 0), TTLT (1) or preemption time (2), their number and sum. */
+int orc_preempt_time(orc_sim* s, int64_t* out) {
+  if (!s || !s->have_reps || !out) return ORC_EINVAL;
+  const int64_t N = s->cfg.max_requests;
+  for (int64_t r = 0; r < s->cfg.n_replicas; r++) {
+    const orc_rep* x = &s->rep[r];
+    const int64_t nreq = s->n_req[x->par.trace_id];
+    for (int64_t i = 0; i < N; i++) out[r * N + i] = i < nreq ? x->req[i].t_preempt : 0;
+  }
+  return ORC_OK;
+}
+
+int orc_class_percentiles(orc_sim* s, int64_t which, int64_t len_lo, int64_t len_hi, const int64_t* permille, int64_t n,
+                          int64_t* out, int64_t* count, int64_t* sum) {
+  if (!s || !s->have_reps || !permille || !out || which < 0 || which > 2 || n < 1) return ORC_EINVAL;
+  const int64_t N = s->cfg.max_requests;
+  int64_t* v = (int64_t*)malloc(sizeof(int64_t) * (size_t)(N > 0 ? N : 1));
+  if (!v) return ORC_ENOMEM;
+  for (int64_t r = 0; r < s->cfg.n_replicas; r++) {
+    const orc_rep* x = &s->rep[r];
+    const int64_t tr = x->par.trace_id, nreq = s->n_req[tr];
+    int64_t m = 0, tot = 0;
+    for (int64_t i = 0; i < nreq; i++) {
+      const orc_req* q = &x->req[i];
+      const int64_t len = (int64_t)s->prompt[tr * N + i] + (int64_t)s->decode[tr * N + i];
+      if (!q->completed || len < len_lo || len > len_hi) continue;
+      const int64_t a = s->arrival[tr * N + i];
+      v[m] = which == 0 ? q->t_first - a : (which == 1 ? q->t_last - a : q->t_preempt);
+      tot += v[m];
+      m++;
+    }
+    qsort(v, (size_t)m, sizeof(int64_t), i64_cmp_);
+    for (int64_t k = 0; k < n; k++) {
+      if (permille[k] < 1 || permille[k] > 1000) { free(v); return ORC_EINVAL; }
+      if (m == 0) { out[r * n + k] = 0; continue; }
+      int64_t rank = (permille[k] * m + 999) / 1000;
+      if (rank < 1) rank = 1;
+      if (rank > m) rank = m;
+      out[r * n + k] = v[rank - 1];
+    }
+    if (count) count[r] = m;
+    if (sum) sum[r] = tot;
   }
   free(v);
   return ORC_OK;

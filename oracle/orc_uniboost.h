@@ -150,6 +150,15 @@ int  orc_digest(orc_sim*, uint64_t* digest /* [R] */);
  * SLO attainment (Fig. 8): number of samples <= threshold, per replica and threshold. */
 int  orc_percentile_curve(orc_sim*, int64_t which, const int64_t* permille /* [n] */, int64_t n, int64_t* out_us /* [R][n] */);
 int  orc_slo_attainment(orc_sim*, int64_t which, const int64_t* threshold_us /* [R][n] */, int64_t n, int64_t* met /* [R][n] */);
+/* Rule M15 ("the preemption time of longer requests", Table 5): a request is
+ * preempted from the start of the iteration that evicts it (swap or recompute) to the start of the iteration that
+ * admits it again; its preemption time is the sum over its evictions.  out: [R][N] microseconds. */
+int  orc_preempt_time(orc_sim*, int64_t* out);
+/* Per-class reductions (Tables 3-5): over the completed requests of a replica whose total
+ * length P + D lies in [len_lo, len_hi]: nearest-rank percentiles at n per-mille points of TTFT (which 0), TTLT (1) or
+ * preemption time (2) -> out [R][n]; their number -> count [R] (nullable); their sum -> sum [R] (nullable). */
+int  orc_class_percentiles(orc_sim*, int64_t which, int64_t len_lo, int64_t len_hi, const int64_t* permille, int64_t n,
+                           int64_t* out, int64_t* count, int64_t* sum);
 int  orc_boost_lut(orc_sim*, int64_t replica, int64_t* lut /* [cap] */, int64_t cap, int64_t* nb);
 int  orc_tbt_hist(orc_sim*, int64_t replica, uint32_t* hist /* [4352] */);
 /* stand-alone helpers exposed so the pins can hit them directly */
