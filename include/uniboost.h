@@ -169,7 +169,8 @@ enum { UB_F_RESIDENT = 1u,        /* KV on the device */
                                      iteration: the only requests that may be out of place in the stored order */
        UB_F_ADMITNOW = 16u,       /* admitted in the last executed iteration */
        UB_F_KLASS1   = 32u,       /* was in class 1 (not MemGuard-locked) in the last executed iteration */
-       UB_F_LOCK_SHIFT = 6 };     /* bits 6..31: MemGuard lock bin + 1 (0 = no lock; residents re-lock every iteration, M10) */
+       UB_F_PREEMPTED = 64u,      /* evicted (swap or recompute) and not admitted again yet (its preemption time is running) */
+       UB_F_LOCK_SHIFT = 7 };     /* bits 7..31: MemGuard lock bin + 1 (0 = no lock; residents re-lock every iteration, M10) */
 
 /* Kernel-level parity (SURVEY.md Sec. 4 tier T1, Sec. 8(b)): overwrite the state of one unfinished replica so that a
  * single ub_step runs admit / victim-select / advance (a3..a5) from a state taken from elsewhere, e.g. an oracle
@@ -209,6 +210,22 @@ int  ub_last_step_timing(ub_sim*, float* kernel_ms, uint32_t* launches);
  * Both synchronise. */
 int  ub_percentile_curve(ub_sim*, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out_us);
 int  ub_slo_attainment(ub_sim*, uint32_t which, const int64_t* threshold_us, uint32_t n, uint32_t* met);
+
+/* Per-class reductions (the short- / long-request tables of the starvation experiment,
+ * PAPER.md:549-560 Table 3, Tables 4-5), device-resident: over the completed requests of each replica
+ * whose total length P + D lies in [len_lo, len_hi], the nearest-rank percentiles (t_p of PAPER.md:225, rank
+ * ceil(p m / 1000); per-mille 1000 = the maximum) at n (1..16) points of
+ *   which 0: TTFT,  1: TTLT (E2E),  2: preemption time -- the time from the start of the iteration that evicts a request
+ *   (swap or recompute) to the start of the iteration that admits it again, summed over its evictions ("the preemption
+ *   time of longer requests"; rule M15 of DESIGN.md).
+ * out_us: host [n_replicas][n] (0 where the class is empty); count: host [n_replicas], requests in the class (nullable);
+ * sum_us: host [n_replicas], sum of their values -- the mean is sum / count (nullable).  Synchronises. */
+int  ub_class_percentiles(ub_sim*, uint32_t which, uint32_t len_lo, uint32_t len_hi, const uint32_t* permille, uint32_t n,
+                          int64_t* out_us, uint32_t* count, int64_t* sum_us);
+/* Preemption time of every request so far (rule M15), [n_replicas][max_requests] microseconds, host (on_device = 0) or
+ * device.  A request that is preempted right now shows minus the start time of its eviction plus the finished part.
+ * Synchronises. */
+int  ub_preempt_time(ub_sim*, int64_t* t_preempt_us, int on_device);
 
 /* gamma-Ada (Eq. 9, UPDATEGAMMA PAPER.md:588-601; rule M13 of DESIGN.md),
  * integer-only so that schedules stay bit-exact.  gamma is kept as gamma_u = gamma * 1e6.  At the start of an executed

@@ -58,6 +58,7 @@ EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_st
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
            "ub_last_step_timing", "ub_set_iters_per_launch", "ub_set_gamma_ada", "ub_gamma_state", "ub_gamma_grid",
            "ub_percentile_curve", "ub_slo_attainment", "ub_debug_keys", "ub_debug_keys_stream", "ub_debug_set_state",
+           "ub_class_percentiles", "ub_preempt_time",
            "ub_strerror")
 
 _lib = None
@@ -92,6 +93,8 @@ def lib():
         L.ub_debug_set_state.argtypes = [vp, U32, U32, vp, vp, vp, vp, I64, U32, U32]
         L.ub_percentile_curve.argtypes = [vp, U32, vp, U32, vp]
         L.ub_slo_attainment.argtypes = [vp, U32, vp, U32, vp]
+        L.ub_class_percentiles.argtypes = [vp, U32, U32, U32, vp, U32, vp, vp, vp]
+        L.ub_preempt_time.argtypes = [vp, vp, C.c_int]
         L.ub_set_gamma_ada.argtypes = [vp, P(UbGammaAda), vp]
         L.ub_gamma_state.argtypes = [vp, U32, P(I64), P(C.c_int32), P(U64)]
         L.ub_gamma_grid.argtypes = [vp, vp]
@@ -284,6 +287,22 @@ class Sim:
         assert thr.ndim == 2 and thr.shape[0] == self.R
         out = np.zeros(thr.shape, np.uint32)
         _chk(lib().ub_slo_attainment(self._h, int(which), thr.ctypes.data, thr.shape[1], out.ctypes.data))
+        return out
+
+    def class_percentiles(self, which, len_lo, len_hi, permille):
+        """(percentiles [R][n] int64 us, count [R], sum [R]) of TTFT (0) / TTLT (1) / preemption time (2) over the completed
+        requests with len_lo <= P + D <= len_hi (ub_class_percentiles)."""
+        pm = np.ascontiguousarray(permille, np.uint32)
+        out = np.zeros((self.R, len(pm)), np.int64); cnt = np.zeros(self.R, np.uint32); tot = np.zeros(self.R, np.int64)
+        hi = min(int(len_hi), 0xFFFFFFFF)
+        _chk(lib().ub_class_percentiles(self._h, int(which), int(len_lo), hi, pm.ctypes.data, len(pm), out.ctypes.data,
+                                        cnt.ctypes.data, tot.ctypes.data))
+        return out, cnt.astype(np.int64), tot
+
+    def preempt_time(self):
+        """[R][N] int64 microseconds each request spent preempted (rule M15)."""
+        out = np.zeros((self.R, self.N), np.int64)
+        _chk(lib().ub_preempt_time(self._h, out.ctypes.data, 0))
         return out
 
     def set_gamma_ada(self, ada: dict, adaptive):

@@ -22,7 +22,7 @@ struct ub_sim {
   bool have_trace, have_reps;
   // owned device memory
   Rec0* d_E0; Rec1* d_E1; Hdr* d_hdr; Rec0* d_TR; uint32_t* d_nreq; int64_t* d_lut;
-  int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
+  int64_t* d_tpre; int64_t* d_tfirst; int64_t* d_tlast; uint32_t* d_ne; uint32_t* d_neu; uint32_t* d_hist;
   StatsDev* d_stats; unsigned long long* d_word;
   uint32_t* d_list; uint32_t* d_count;   // work lists [4][R]; counts [8] ([5] = finished replicas)
   uint32_t* d_live; uint32_t* d_livecnt; // ub_run's tail: the unfinished replicas of each part of a round, compacted
@@ -97,7 +97,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
   int rc = UB_OK;
   if ((rc = dmalloc(&s->d_E0, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_E1, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_hdr, R)) ||
       (rc = dmalloc(&s->d_nreq, NT)) || (rc = dmalloc(&s->d_tfirst, R * N)) ||
-      (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
+      (rc = dmalloc(&s->d_tlast, R * N)) || (rc = dmalloc(&s->d_tpre, R * N)) || (rc = dmalloc(&s->d_ne, R * N)) || (rc = dmalloc(&s->d_neu, R * N)) ||
       (rc = dmalloc(&s->d_hist, R * (size_t)kTbtBins)) || (rc = dmalloc(&s->d_stats, R)) ||
       (rc = dmalloc(&s->d_word, 2)) || (rc = dmalloc(&s->d_live, R)) || (rc = dmalloc(&s->d_livecnt, kMaxSplit + 1)) ||
       (rc = dmalloc(&s->d_drift, R)) || (rc = dmalloc(&s->d_drift_live, R)) || (rc = dmalloc(&s->d_list, 4 * kMaxSplit * R)) || (rc = dmalloc(&s->d_count, 8 * kMaxSplit)) ||
@@ -129,7 +129,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
   d.k = c->bin_tokens; d.c0 = c->c0_us; d.c_pf = c->c_prefill_tok_us; d.c_dec = c->c_decode_seq_us;
   d.E0 = s->d_E0; d.E1 = s->d_E1; d.hdr = s->d_hdr; d.n_req = s->d_nreq;
   d.evbuf = s->d_evbuf; d.evcap = c->max_batch < c->queue_cap ? c->max_batch : c->queue_cap;
-  d.t_first = s->d_tfirst; d.t_last = s->d_tlast; d.n_evict = s->d_ne; d.n_evict_unf = s->d_neu; d.hist = s->d_hist;
+  d.t_first = s->d_tfirst; d.t_last = s->d_tlast; d.t_pre = s->d_tpre; d.n_evict = s->d_ne; d.n_evict_unf = s->d_neu; d.hist = s->d_hist;
   *out = s;
   return UB_OK;
 }
@@ -139,7 +139,7 @@ void ub_destroy(ub_sim* s) {
   cudaSetDevice(s->cfg.device);
   cudaStreamSynchronize(s->stream);
   cudaFree(s->d_E0); cudaFree(s->d_E1); cudaFree(s->d_hdr); cudaFree(s->d_TR);
-  cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_ne);
+  cudaFree(s->d_nreq); cudaFree(s->d_lut); cudaFree(s->d_tfirst); cudaFree(s->d_tlast); cudaFree(s->d_tpre); cudaFree(s->d_ne);
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
   cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_evbuf); cudaFree(s->d_live); cudaFree(s->d_livecnt); cudaFree(s->d_drift); cudaFree(s->d_drift_live);
   cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);
@@ -313,6 +313,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   // reset the run state
   CK(cudaMemsetAsync(s->d_tfirst, 0xFF, R * N * 8, s->stream));     // -1
   CK(cudaMemsetAsync(s->d_tlast, 0xFF, R * N * 8, s->stream));
+  CK(cudaMemsetAsync(s->d_tpre, 0, R * N * 8, s->stream));
   CK(cudaMemsetAsync(s->d_ne, 0, R * N * 4, s->stream));
   CK(cudaMemsetAsync(s->d_neu, 0, R * N * 4, s->stream));
   CK(cudaMemsetAsync(s->d_hist, 0, R * (size_t)kTbtBins * 4, s->stream));
@@ -652,6 +653,39 @@ int ub_percentile_curve(ub_sim* s, uint32_t which, const uint32_t* permille, uin
   if (e == cudaSuccess) e = cudaGetLastError();
   cudaFree(d_out);
   if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  return UB_OK;
+}
+
+int ub_class_percentiles(ub_sim* s, uint32_t which, uint32_t len_lo, uint32_t len_hi, const uint32_t* permille, uint32_t n,
+                         int64_t* out, uint32_t* count, int64_t* sum) {
+  if (!s || !permille || !out || which > 2 || n < 1 || n > 16 || len_lo > len_hi) return UB_EINVAL;
+  for (uint32_t k = 0; k < n; k++) if (permille[k] < 1 || permille[k] > 1000) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t R = s->cfg.n_replicas;
+  int64_t* d_out = nullptr; uint32_t* d_cnt = nullptr; int64_t* d_sum = nullptr;
+  int rc = UB_OK;
+  if ((rc = dmalloc(&d_out, R * n)) || (rc = dmalloc(&d_cnt, R)) || (rc = dmalloc(&d_sum, R))) {
+    cudaFree(d_out); cudaFree(d_cnt); cudaFree(d_sum); return rc;
+  }
+  launch_class_percentiles(s->dev, which, len_lo, len_hi, permille, n, d_out, d_cnt, d_sum, s->stream);
+  cudaError_t e = cudaMemcpyAsync(out, d_out, R * n * 8, cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess && count) e = cudaMemcpyAsync(count, d_cnt, R * 4, cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess && sum) e = cudaMemcpyAsync(sum, d_sum, R * 8, cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  cudaFree(d_out); cudaFree(d_cnt); cudaFree(d_sum);
+  if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  return UB_OK;
+}
+
+int ub_preempt_time(ub_sim* s, int64_t* out, int on_device) {
+  if (!s || !out) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t tot = (size_t)s->cfg.n_replicas * s->cfg.max_requests;
+  CK(cudaMemcpyAsync(out, s->d_tpre, tot * 8, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->stream));
+  CK(cudaStreamSynchronize(s->stream));
   return UB_OK;
 }
 

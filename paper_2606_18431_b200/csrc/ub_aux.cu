@@ -318,6 +318,88 @@ void launch_percentile_curve(const SimDev& s, uint32_t which, const uint32_t* pe
   k_percentile_curve<<<s.R, kStatThreads, 0, st>>>(s, c, out);
 }
 
+// Per-class reductions (Tables 3-5): over the completed requests of a replica whose total
+// length P + D lies in [len_lo, len_hi] -- the paper's short / long split -- nearest-rank percentiles of TTFT (which 0),
+// TTLT (1) or preemption time (2, rule M15), their number and their sum.  The same MSD radix select as a6, with the
+// class filter and the value folded into the scan.
+struct ClassArgs { uint32_t which, n, len_lo, len_hi; uint32_t permille[16]; };
+__global__ void __launch_bounds__(kStatThreads) k_class_percentiles(SimDev s, ClassArgs c, int64_t* out, uint32_t* count,
+                                                                    int64_t* sum) {
+  __shared__ SelectSmem sm;
+  __shared__ unsigned long long tot_sum;
+  __shared__ uint32_t tot_cnt;
+  const uint32_t r = blockIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t tr = s.hdr[r].par.trace_id, nreq = s.n_req[tr];
+  const Rec0* TR = s.TR + (size_t)tr * s.N;
+  const int64_t* src = (c.which == 0 ? s.t_first : (c.which == 1 ? s.t_last : s.t_pre)) + (size_t)r * s.N;
+  const uint32_t* ne = s.n_evict + (size_t)r * s.N;
+  // value of request i if it belongs to the class
+  auto value = [&](uint32_t i, unsigned long long& v) -> bool {
+    if (!(ne[i] & kDoneBit)) return false;
+    const Rec0 q = TR[i];
+    const uint32_t len = q.P + q.D;
+    if (len < c.len_lo || len > c.len_hi) return false;
+    v = (unsigned long long)(c.which == 2 ? src[i] : src[i] - q.a);
+    return true;
+  };
+  if (tid == 0) { tot_sum = 0ull; tot_cnt = 0u; }
+  __syncthreads();
+  {
+    unsigned long long ls = 0; uint32_t lc = 0;
+    for (uint32_t i = tid; i < nreq; i += kStatThreads) { unsigned long long v; if (value(i, v)) { ls += v; lc++; } }
+    for (int o = 16; o > 0; o >>= 1) { ls += __shfl_xor_sync(0xffffffffu, ls, o); lc += __shfl_xor_sync(0xffffffffu, lc, o); }
+    if (lane == 0) { atomicAdd(&tot_sum, ls); atomicAdd(&tot_cnt, lc); }
+  }
+  __syncthreads();
+  const uint32_t m = tot_cnt;
+  if (tid == 0) { if (count) count[r] = m; if (sum) sum[r] = (int64_t)tot_sum; }
+  for (uint32_t k = 0; k < c.n; k++) {
+    int64_t result = 0;
+    if (m > 0) {
+      uint64_t rank = ((uint64_t)c.permille[k] * m + 999) / 1000;
+      if (rank < 1) rank = 1;
+      if (rank > m) rank = m;
+      // MSD radix select of the (rank-1)-th smallest class value, 8 passes of 8 bits
+      if (tid == 0) { sm.prefix = 0ull; sm.rank = (uint32_t)(rank - 1); }
+      for (int pass = 7; pass >= 0; pass--) {
+        sm.hist[tid] = 0;
+        __syncthreads();
+        const unsigned long long prefix = sm.prefix;
+        const int sh_hi = 8 * (pass + 1);
+        for (uint32_t i = tid; i < nreq; i += kStatThreads) {
+          unsigned long long v;
+          if (!value(i, v)) continue;
+          if (pass == 7 || (v >> sh_hi) == (prefix >> sh_hi)) atomicAdd(&sm.hist[(v >> (8 * pass)) & 0xFF], 1u);
+        }
+        __syncthreads();
+        const uint32_t cntb = sm.hist[tid];
+        uint32_t inc = cntb;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += x; }
+        if (lane == 31) sm.wtot[warp] = inc;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int w = 0; w < warp; w++) off += sm.wtot[w];
+        inc += off;
+        const uint32_t exc = inc - cntb, want = sm.rank;
+        __syncthreads();
+        if (want >= exc && want < inc) { sm.prefix = prefix | ((unsigned long long)tid << (8 * pass)); sm.rank = want - exc; }
+        __syncthreads();
+      }
+      result = (int64_t)sm.prefix;
+      __syncthreads();
+    }
+    if (tid == 0) out[(size_t)r * c.n + k] = result;
+  }
+}
+void launch_class_percentiles(const SimDev& s, uint32_t which, uint32_t len_lo, uint32_t len_hi, const uint32_t* permille,
+                              uint32_t n, int64_t* out, uint32_t* count, int64_t* sum, cudaStream_t st) {
+  ClassArgs c; c.which = which; c.n = n; c.len_lo = len_lo; c.len_hi = len_hi;
+  for (uint32_t k = 0; k < 16; k++) c.permille[k] = k < n ? permille[k] : 0;
+  k_class_percentiles<<<s.R, kStatThreads, 0, st>>>(s, c, out, count, sum);
+}
+
 // SLO attainment (Fig. 8): per replica and threshold, the number of completed requests whose
 // latency is <= the threshold (the caller forms thresholds = SLO scale x base latency).  thr: [R][n] device.
 __global__ void __launch_bounds__(kStatThreads) k_slo_count(SimDev s, uint32_t which, uint32_t n, const int64_t* thr,

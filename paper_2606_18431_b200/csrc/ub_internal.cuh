@@ -29,7 +29,9 @@ constexpr uint32_t F_EMITPREV = 4u;        // emitted a token in the previous ex
 constexpr uint32_t F_DIRTY    = 8u;        // (class,key) may differ from the previous iteration's => listed in dlist
 constexpr uint32_t F_ADMITNOW = 16u;       // admitted in the last executed iteration (read by the eviction pass only)
 constexpr uint32_t F_KLASS1   = 32u;       // was in class 1 (not MemGuard-locked) in the last executed iteration
-constexpr int      F_LOCK_SHIFT = 6;       // bits 6..31: lockbin + 1 (0 = no lock)
+constexpr uint32_t F_PREEMPTED = 64u;      // evicted (swap or recompute) and not yet admitted again (rule M15: preemption time)
+constexpr uint32_t F_PARKED  = F_SWAPPED | F_PREEMPTED;   // what a waiting request may carry besides F_KLASS1
+constexpr int      F_LOCK_SHIFT = 7;       // bits 7..31: lockbin + 1 (0 = no lock)
 constexpr uint32_t F_LOCK_MASK_LOW = (1u << F_LOCK_SHIFT) - 1u;   // the flag bits below the lock field
 constexpr uint32_t kDirtyMax  = 32;        // entries of a replica's dirty list; Hdr::n_dirty > kDirtyMax = overflow
 
@@ -81,6 +83,7 @@ struct SimDev {                 // kernel argument (by value)
   const uint32_t* n_req;        // [NT]
   const int64_t* lut;
   int64_t* t_first; int64_t* t_last;      // [R][N]
+  int64_t* t_pre;                         // [R][N] preemption time (M15): minus the eviction times plus the re-admission times
   uint32_t* n_evict; uint32_t* n_evict_unf;
   uint32_t* hist;               // [R][kTbtBins]
   uint2*    evbuf;              // [R][evcap] scratch: per-request events of one iteration that wait for t_end
@@ -116,6 +119,8 @@ struct StatsDev {               // device-side result of the percentile reductio
 void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st);
 void launch_percentile_curve(const SimDev& s, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out,
                              cudaStream_t st);
+void launch_class_percentiles(const SimDev& s, uint32_t which, uint32_t len_lo, uint32_t len_hi, const uint32_t* permille,
+                              uint32_t n, int64_t* out, uint32_t* count, int64_t* sum, cudaStream_t st);
 void launch_slo_count(const SimDev& s, uint32_t which, uint32_t n, const int64_t* thr, uint32_t* out, cudaStream_t st);
 
 }  // namespace ub

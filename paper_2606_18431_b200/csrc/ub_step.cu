@@ -158,6 +158,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
   const uint32_t ncomp0 = s.ada_ring ? s.hdr[r].n_completed : 0u;     // (gamma-Ada runs one iteration per launch)
   int64_t* g_tfirst = s.t_first + (size_t)r * s.N;
   int64_t* g_tlast = s.t_last + (size_t)r * s.N;
+  int64_t* g_tpre = s.t_pre + (size_t)r * s.N;
   uint32_t* g_hist = s.hist + (size_t)r * kTbtBins;
   uint32_t* g_ne = s.n_evict + (size_t)r * s.N;          // bit 31 = completed marker (read by the stats kernel)
   uint32_t* g_neu = s.n_evict_unf + (size_t)r * s.N;
@@ -544,10 +545,11 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         const uint32_t of = r1[c].flags;
         const uint32_t klass = (of & F_DIRTY) ? 1u : 0u;
         const uint32_t d_old = r1[c].d;
-        uint32_t nf = of & (F_RESIDENT | F_SWAPPED | F_EMITPREV);
+        uint32_t nf = of & (F_RESIDENT | F_SWAPPED | F_EMITPREV | F_PREEMPTED);
         const uint32_t id = r1[c].id;
         if (want[c]) {
-          nf = (nf | F_RESIDENT) & ~F_SWAPPED;
+          if (nf & F_PREEMPTED) g_tpre[id] = __ldcg(g_tpre + id) + t;           // M15: the preemption ends where this iteration starts
+          nf = (nf | F_RESIDENT) & ~(F_SWAPPED | F_PREEMPTED);
           r1[c].cached += want[c];
           if (r1[c].cached == r0[c].P + d_old) {               // KV caught up => one token out (M2)
             r1[c].d = d_old + 1; tot2[0]++;
@@ -578,8 +580,9 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
           }
         } else {
           if (nf & F_EMITPREV) { g_tlast[id] = t; nf &= ~F_EMITPREV; }   // persist t_last when the streak ends
-          if (evm[c] == 1) { r1[c].cached = 0; nf &= ~F_RESIDENT; }
-          else if (evm[c] == 2) { nf = (nf | F_SWAPPED) & ~F_RESIDENT; }
+          if (evm[c] == 1) { r1[c].cached = 0; nf = (nf | F_PREEMPTED) & ~F_RESIDENT; }
+          else if (evm[c] == 2) { nf = (nf | F_SWAPPED | F_PREEMPTED) & ~F_RESIDENT; }
+          if (evm[c]) g_tpre[id] = __ldcg(g_tpre + id) - t;                     // M15: preempted from the start of this iteration on
         }
         // re-lock at this iteration's bin (M10, G6) and leave the dirty hint for the next iteration's ordering:
         // set when (resident, bin, class) -- the inputs of a BOOST / FCFS key -- change.  SRPT / LAS keys move by

@@ -391,9 +391,13 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
           evl += adm ? (uint32_t)h : 0u;
           evu += adm ? (uint32_t)(h >> 32) : 0u;
         }
-        const bool swp = adm && (of & F_SWAPPED);
-        if (__any_sync(kFull, swp)) {                                 // swap-in on admission (rare)
-          if (swp) {
+        const bool back = adm && (of & F_PREEMPTED);
+        if (__any_sync(kFull, back)) {                                // back on the device after an eviction (rare)
+          if (back) {                                                 // M15: the preemption ends where this iteration starts
+            int64_t* g_tp = s.t_pre + (size_t)r * s.N + w1.id;
+            *g_tp = __ldcg(g_tp) + (int64_t)sh[0];
+          }
+          if (back && (of & F_SWAPPED)) {                             // swap-in on admission
             const uint32_t blocks = (w1.cached + blk_m1) >> blk_sh;
             atomicAdd(&X.skb[0].w, blocks); atomicAdd(&X.skb[1].w, 1u);
             ev_add(evl, evu, EV_SWAPIN, w1.id, blocks);
@@ -411,7 +415,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         de += emitted ? 0x10000u : 0u;
         ps += (emitted && d_old != 0u && ep_old) ? 0x10000u : 0u;     // gap == this iteration's cost
         const bool gone = emitted && d2 == w0.D;                      // complete: KV freed at once
-        uint32_t nf = of & (F_RESIDENT | F_SWAPPED);
+        uint32_t nf = of & (F_RESIDENT | F_SWAPPED | F_PREEMPTED);
         if (adm) nf = F_RESIDENT | F_ADMITNOW;
         if (emitted) nf |= F_EMITPREV;
         // re-lock at this iteration's bin (M10, G6); a request is dirty for the next iteration's ordering when
@@ -509,7 +513,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
               // ... optionally followed, when nothing is parked, by steadily waiting requests (not resident, nothing
               // to finalise) whose first one is turned away -- on KV ("newblocked": the walk goes on over residents
               // only, of which this chunk has none left) or because the batch / token budget is used up (walk stops)
-              const bool okw = !okl && (fl & ~F_SWAPPED) == F_KLASS1;
+              const bool okw = !okl && (fl & ~F_PARKED) == F_KLASS1;
               const uint32_t decm = __ballot_sync(kFull, valid && okl);
               const uint32_t wm = pend ? 0u : __ballot_sync(kFull, valid && okw);
               if ((decm | wm) != cv || cv == 0u || (wm != 0u && decm >= (wm & (0u - wm)))) break;   // (decoders first)
@@ -559,7 +563,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
             const uint32_t fl = reinterpret_cast<const uint32_t*>(st + 32 + lane)[3];
             const uint32_t left = n_old - c * 32u;
             const bool valid = (uint32_t)lane < left;
-            if (!__all_sync(kFull, (fl & ~F_SWAPPED) == F_KLASS1 || !valid)) break;
+            if (!__all_sync(kFull, (fl & ~F_PARKED) == F_KLASS1 || !valid)) break;
             const uint32_t np = outpos + (uint32_t)lane;
             if (outpos != c * 32u && valid) {
               const uint4 c0 = st[lane], c1 = st[32 + lane];
@@ -586,7 +590,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         if (mode != 0u && cv != 0u && !drift) {
           // ---- behind the walk: a chunk of waiting requests (not resident, nothing to finalise) that sorts in front
           // of the next parked request, if any, only moves up
-          const bool steady = (r1.flags & ~F_SWAPPED) == F_KLASS1;
+          const bool steady = (r1.flags & ~F_PARKED) == F_KLASS1;
           if (__all_sync(kFull, steady || !((cv >> lane) & 1u))) {
             bool before = true;
             if (dptr < m) {
@@ -707,16 +711,18 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
             if (do_swap) {
               swap_used += resb; swout_blocks += resb; ev_nsw++;
               if (lane == 0) ev_add(evl, evu, EV_EVICT_SWAP, id_l, resb);
-              if (lane == l) q.flags = F_SWAPPED | F_DIRTY;
+              if (lane == l) q.flags = F_SWAPPED | F_PREEMPTED | F_DIRTY;
             } else {
               ev_lost += cached_l; ev_nrc++;
               if (lane == 0) ev_add(evl, evu, EV_EVICT_RECOMPUTE, id_l, cached_l);
-              if (lane == l) { q.cached = 0; q.flags = F_DIRTY; }
+              if (lane == l) { q.cached = 0; q.flags = F_PREEMPTED | F_DIRTY; }
             }
           }
           if (victim) {
             uint32_t* g_ne = s.n_evict + (size_t)r * s.N;
             g_ne[q.id] = __ldcg(g_ne + q.id) + 1u;
+            int64_t* g_tp = s.t_pre + (size_t)r * s.N + q.id;         // M15: preempted from the start of this iteration on
+            *g_tp = __ldcg(g_tp) - (int64_t)sh[0];
             if (of & F_KLASS1) {                                      // victim was not MemGuard-locked
               uint32_t* g_neu = s.n_evict_unf + (size_t)r * s.N;
               g_neu[q.id] = __ldcg(g_neu + q.id) + 1u;

@@ -17,7 +17,7 @@ from tests.helpers import pressure_workload
 
 pytestmark = pytest.mark.gpu
 
-F_RESIDENT, F_SWAPPED, F_EMITPREV, F_DIRTY, F_ADMITNOW, F_KLASS1, F_LOCK_SHIFT = 1, 2, 4, 8, 16, 32, 6
+F_RESIDENT, F_SWAPPED, F_EMITPREV, F_DIRTY, F_ADMITNOW, F_KLASS1, F_PREEMPTED, F_LOCK_SHIFT = 1, 2, 4, 8, 16, 32, 64, 7
 
 
 @pytest.fixture(scope="module")
@@ -89,9 +89,10 @@ class _Tracker:
                 swapped = False
             else:
                 swapped = q["swapped"]
+            preempted = bool(r["evict"]) or (q.get("preempted", False) and r["want"] == 0)
             self.req[i] = dict(d=r["d_after"], cached=r["cached_after"], resident=bool(r["resident_after"]),
                                swapped=swapped, emitted=emitted, admitted=r["want"] > 0, klass=r["klass"], bin=r["bin"],
-                               res_before=bool(r["resident_before"]))
+                               res_before=bool(r["resident_before"]), preempted=preempted)
             self.next = max(self.next, i + 1)
             if r["d_after"] < self.D[i]:
                 new_order.append(i)
@@ -114,6 +115,8 @@ class _Tracker:
                 f |= F_RESIDENT | ((q["bin"] + 1) << F_LOCK_SHIFT)
             if q["swapped"]:
                 f |= F_SWAPPED
+            if q["preempted"]:
+                f |= F_PREEMPTED
             if q["emitted"]:
                 f |= F_EMITPREV
             if q["admitted"]:
