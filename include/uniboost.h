@@ -43,9 +43,13 @@ enum { UB_OK = 0, UB_EINVAL = -1, UB_ENOMEM = -2, UB_ECUDA = -3, UB_ESTATE = -4,
 enum { UB_FCFS = 0, UB_SRPT = 1, UB_BOOST = 2, UB_LAS = 3,
        UB_SJF = 4,    /* shortest job first: key = hidden output length D (perfect lengths) */
        UB_SPF = 5,    /* shortest prompt first: key = prompt length P */
-       UB_DISTBOOST = 6 };  /* Phase-1 strawman DistBoost: decode queue first, keyed by the time of
+       UB_DISTBOOST = 6,    /* Phase-1 strawman DistBoost: decode queue first, keyed by the time of
                                entering it (Eq. 4); prefill queue keyed by a - b_gamma(prompt) (Eq. 3); guard and
                                hysteresis are not applied */
+       UB_SARATHI = 7 };    /* the Sarathi baseline ("chunk-prefill, decode-prioritized continuous batching,
+                               with round-robin ordering in the decode and piggy-back prefills"; rule M16): decode queue
+                               first, ordered by the time of the request's last token; prefill queue first come first
+                               served; guard and hysteresis are not applied */
 /* size signal (M3): P+d | SIGNAL of PAPER.md:575-587 | D-d (tests: SRPT limit) */
 enum { UB_SIG_UNIFIED = 0, UB_SIG_PHASE = 1, UB_SIG_REMAINING = 2 };
 /* quantiser (M3): Eq. 8 geometric bins | identity (vanilla boost, tests) */
@@ -85,7 +89,7 @@ typedef struct {
 /* One per replica: policies / gamma points / trace seeds run side by side as the batch dimension. */
 typedef struct {
   uint32_t trace_id;
-  uint8_t  policy;                /* UB_FCFS .. UB_DISTBOOST */
+  uint8_t  policy;                /* UB_FCFS .. UB_SARATHI */
   uint8_t  guard;                 /* MemGuard lock on/off */
   uint8_t  signal_mode;           /* UB_SIG_* */
   uint8_t  quant_mode;            /* UB_Q_* */

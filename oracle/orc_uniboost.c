@@ -215,7 +215,7 @@ int orc_set_replicas(orc_sim* s, const orc_replica* reps) {
   for (int64_t r = 0; r < R; r++) {
     const orc_replica* q = &reps[r];
     if (q->trace_id < 0 || q->trace_id >= c->n_traces) return ORC_EINVAL;
-    if (q->policy < 0 || q->policy > 6 || q->signal_mode < 0 || q->signal_mode > 2 ||
+    if (q->policy < 0 || q->policy > 7 || q->signal_mode < 0 || q->signal_mode > 2 ||
         q->quant_mode < 0 || q->quant_mode > 1 || q->hysteresis_us < 0 ||
         q->hysteresis_us > ((int64_t)1 << 60))
       return ORC_EINVAL;
@@ -429,13 +429,19 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
         key = A[id] - x->lut[pb < x->nb ? pb : x->nb - 1];
       }
     }
+    else if (x->par.policy == ORC_SARATHI) {
+      /* Sarathi (M16; "chunk-prefill, decode-prioritized continuous batching, with round-robin ordering in the decode
+         and piggy-back prefills"): the decode queue goes round robin -- whoever emitted longest ago
+         first --, the prefill queue is first come first served */
+      key = (q->d >= 1) ? q->t_last : A[id];
+    }
     else key = A[id] - x->lut[bin < x->nb ? bin : x->nb - 1];
     /* Eq. 7 hysteresis as a bias on requests that hold the device */
     if (q->resident && (x->par.policy == ORC_FCFS || x->par.policy == ORC_BOOST)) key -= x->par.hysteresis_us;
     /* MemGuard minimum-run lock: dispatched and still in the bin it was locked at */
     int64_t klass = (x->par.guard && q->resident && bin == q->lockbin) ? 0 : 1;
     /* DistBoost: the decode batch is selected first, prefill piggybacks on what is left (Eq. 5-6) */
-    if (x->par.policy == ORC_DISTBOOST) klass = (q->d >= 1) ? 0 : 1;
+    if (x->par.policy == ORC_DISTBOOST || x->par.policy == ORC_SARATHI) klass = (q->d >= 1) ? 0 : 1;
     e[j].klass = klass; e[j].key = key; e[j].id = id; e[j].bin = bin;
     e[j].resident_before = q->resident; e[j].want = 0; e[j].evict = 0;
   }

@@ -54,7 +54,8 @@ extern "C" {
 
 /* policies (M5) */
 enum { ORC_FCFS = 0, ORC_SRPT = 1, ORC_BOOST = 2, ORC_LAS = 3, ORC_SJF = 4, ORC_SPF = 5,
-       ORC_DISTBOOST = 6 };  /* Phase-1 strawman, PAPER.md:150-175 (rule M14) */
+       ORC_DISTBOOST = 6,    /* Phase-1 strawman, PAPER.md:150-175 (rule M14) */
+       ORC_SARATHI = 7 };    /* decode-prioritised, round-robin decode, FCFS chunked prefill piggy-backing (rule M16) */
 /* size signal (M3) */
 enum { ORC_SIG_UNIFIED = 0, ORC_SIG_PHASE = 1, ORC_SIG_REMAINING = 2 };
 /* quantiser (M3) */

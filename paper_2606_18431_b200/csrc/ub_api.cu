@@ -234,7 +234,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   bool any_exact = false;
   for (size_t r = 0; r < R; r++) {
     const ub_replica& q = reps[r];
-    if (q.trace_id >= c.n_traces || q.policy > 6 || q.signal_mode > 2 || q.quant_mode > 1 || q.guard > 1 ||
+    if (q.trace_id >= c.n_traces || q.policy > 7 || q.signal_mode > 2 || q.quant_mode > 1 || q.guard > 1 ||
         q.hysteresis_us < 0 || q.hysteresis_us > (1ll << 60))
       return UB_EINVAL;
     if ((q.policy == UB_BOOST || q.policy == UB_DISTBOOST) && !(q.gamma > 0.0)) return UB_EINVAL;     // also rejects NaN
@@ -289,7 +289,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   {
     bool all = s->dev.blk_shift < 32u;
     for (size_t r = 0; r < R && all; r++)
-      all = reps[r].policy != UB_DISTBOOST && reps[r].signal_mode == 0 && reps[r].quant_mode == 0;
+      all = reps[r].policy < UB_DISTBOOST && reps[r].signal_mode == 0 && reps[r].quant_mode == 0;
     s->dev.all_stream = all ? 1u : 0u;
   }
   {
@@ -790,7 +790,7 @@ __global__ void k_debug_keys(SimDev s, uint32_t r, uint32_t n, uint32_t* id, uns
     const Rec0 q0 = s.E0[(size_t)r * s.Q + p];
     const Rec1 q1 = s.E1[(size_t)r * s.Q + p];
     id[p] = q1.id;
-    okey[p] = okey_of(s, par, lut, tfirst, q0, q1);
+    okey[p] = okey_of(s, par, lut, tfirst, s.t_last + (size_t)r * s.N, s.hdr[r].t, q0, q1);
   }
 }
 
@@ -800,7 +800,7 @@ static int debug_keys_impl(ub_sim* s, uint32_t r, uint32_t* n_active, uint32_t* 
   if (!s->have_reps) return UB_ESTATE;
   if (stream_scorer) {                             // the streaming kernel covers FCFS / BOOST with the paper's signal and quantiser
     const ub_replica& q = s->h_reps[r];
-    if (q.policy == UB_DISTBOOST || q.signal_mode != UB_SIG_UNIFIED || q.quant_mode != UB_Q_GEOMETRIC || s->dev.blk_shift >= 32u)
+    if (q.policy >= UB_DISTBOOST || q.signal_mode != UB_SIG_UNIFIED || q.quant_mode != UB_Q_GEOMETRIC || s->dev.blk_shift >= 32u)
       return UB_EINVAL;
   }
   if (set_dev(s)) return UB_ECUDA;

@@ -57,9 +57,10 @@ __device__ __forceinline__ uint32_t bin_of(const RepPar& par, uint32_t k, uint32
 
 // a1 for every policy (M3-M5, M14): okey = class<<63 | (key + 2^62) of one request; the general form used by the team
 // kernels and by ub_debug_keys (the streaming kernel has its own lean copy for FCFS / BOOST, ub_stream.cu score()).
-// lut: the replica's boost table (already offset by its gamma-Ada level); tfirst: the replica's t_first row.
+// lut: the replica's boost table (already offset by its gamma-Ada level); tfirst / tlast: the replica's t_first / t_last
+// rows; t: the replica clock (a request that emitted in the last iteration carries its t_last implicitly: == t).
 __device__ __forceinline__ uint64_t okey_of(const SimDev& s, const RepPar& par, const int64_t* lut, const int64_t* tfirst,
-                                            const Rec0& q0, const Rec1& q1) {
+                                            const int64_t* tlast, const int64_t t, const Rec0& q0, const Rec1& q1) {
   const uint32_t sig = signal_of(par, q0.P, q0.D, q1.d);
   const uint32_t bin = bin_of(par, s.k, sig);
   int64_t kv;
@@ -72,11 +73,15 @@ __device__ __forceinline__ uint64_t okey_of(const SimDev& s, const RepPar& par, 
     if (q1.d >= 1u) kv = __ldcg(tfirst + q1.id);
     else { const uint32_t pb = bin_of(par, s.k, q0.P); kv = q0.a - __ldg(lut + (pb < par.lut_nb ? pb : par.lut_nb - 1)); }
   }
+  else if (par.policy == 7) {                                                      // Sarathi (M16)
+    // decode queue round robin: by the time of the last token; prefill queue first come first served
+    kv = q1.d >= 1u ? ((q1.flags & F_EMITPREV) ? t : __ldcg(tlast + q1.id)) : q0.a;
+  }
   else kv = q0.a - __ldg(lut + (bin < par.lut_nb ? bin : par.lut_nb - 1));         // pi = a - b
   const bool res = (q1.flags & F_RESIDENT) != 0;
   if (res && (par.policy == 0 || par.policy == 2)) kv -= par.delta;                // Eq. 7 as a bias
   uint64_t klass = (par.guard && res && (q1.flags >> F_LOCK_SHIFT) == bin + 1u) ? 0ull : 1ull;   // MemGuard lock
-  if (par.policy == 6) klass = q1.d >= 1u ? 0ull : 1ull;                           // decode batch first, Eq. 5-6
+  if (par.policy == 6 || par.policy == 7) klass = q1.d >= 1u ? 0ull : 1ull;        // decode batch first, Eq. 5-6 / PAPER.md:239
   return (klass << 63) | (uint64_t)(kv + kKeyBias);
 }
 

@@ -245,7 +245,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
       const uint32_t pos = c * TH + tid;
       key[c] = ~0ull;
       if (pos < n) {
-        key[c] = okey_of(s, par, lut, g_tfirst, r0[c], r1[c]);
+        key[c] = okey_of(s, par, lut, g_tfirst, g_tlast, t, r0[c], r1[c]);
         const uint64_t klass = key[c] >> 63;
         const uint32_t dirty = (r1[c].flags & F_DIRTY) ? 1u : 0u;
         n_dirty += dirty;
@@ -593,7 +593,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
         if (r1[c].d != d_old) bin2 = bin_of(par, s.k, signal_of(par, r0[c].P, r0[c].D, r1[c].d));
         const bool res2 = (nf & F_RESIDENT) != 0;
         uint32_t klass2 = (par.guard && res2 && bin2 == bin) ? 0u : 1u;
-        if (par.policy == 6) klass2 = r1[c].d >= 1u ? 0u : 1u;                         // DistBoost: phase = class
+        if (par.policy == 6 || par.policy == 7) klass2 = r1[c].d >= 1u ? 0u : 1u;      // DistBoost, Sarathi: phase = class
         const bool bin_matters = par.policy == 2;
         const bool dirty = (((nf ^ of) & F_RESIDENT) != 0) || (bin_matters && bin2 != bin) || (klass2 != klass);
         if (res2) nf |= (bin + 1u) << F_LOCK_SHIFT;

@@ -27,7 +27,7 @@ from typing import Callable, Dict, List, Optional, Sequence
 
 import numpy as np
 
-POLICY_FCFS, POLICY_SRPT, POLICY_BOOST, POLICY_LAS, POLICY_SJF, POLICY_SPF, POLICY_DISTBOOST = 0, 1, 2, 3, 4, 5, 6
+POLICY_FCFS, POLICY_SRPT, POLICY_BOOST, POLICY_LAS, POLICY_SJF, POLICY_SPF, POLICY_DISTBOOST, POLICY_SARATHI = 0, 1, 2, 3, 4, 5, 6, 7
 SIG_UNIFIED, SIG_PHASE, SIG_REMAINING = 0, 1, 2
 QUANT_GEOMETRIC, QUANT_EXACT = 0, 1
 PRE_RECOMPUTE, PRE_SWAP, PRE_AUTO = 0, 1, 2

@@ -135,7 +135,7 @@ def test_config1_step_by_step(gpu, oracle_mod):
 # ------------------------------------------------------------------------------------------ memory pressure
 
 @pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS, W.POLICY_SJF,
-                                    W.POLICY_SPF, W.POLICY_DISTBOOST])
+                                    W.POLICY_SPF, W.POLICY_DISTBOOST, W.POLICY_SARATHI])
 @pytest.mark.parametrize("preempt", [W.PRE_RECOMPUTE, W.PRE_SWAP, W.PRE_AUTO])
 def test_pressure_policies_preemption(gpu, oracle_mod, policy, preempt):
     for seed in range(4):
@@ -383,7 +383,7 @@ def test_stream_path_randomised(gpu, oracle_mod, seed):
 # ------------------------------------------------------------------------------------------ kernel-level parity: a1 score
 
 @pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS, W.POLICY_SJF,
-                                    W.POLICY_SPF, W.POLICY_DISTBOOST])
+                                    W.POLICY_SPF, W.POLICY_DISTBOOST, W.POLICY_SARATHI])
 def test_score_kernel_keys_match_oracle(gpu, oracle_mod, policy):
     """SURVEY.md Sec. 4 tier T1: before every iteration the (class, key) the device assigns to each request of the
     window (ub_debug_keys, the team kernels' own scoring function) equals what the oracle scores in that iteration."""

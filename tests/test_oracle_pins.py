@@ -716,3 +716,78 @@ def test_distboost_two_queues_eq3_to_eq6():
     tf = o.per_request()[0][0]
     assert all(tf[i] == t for i, t in first.items())
     o.close()
+
+
+# ------------------------------------------------------------------ M16 Sarathi
+
+@pytest.mark.parametrize("seed", range(4))
+def test_sarathi_single_slot_is_non_preemptive_fifo(seed):
+    """Decode-prioritised: with one slot and one-token prompts a request that has started decoding holds
+    the server until it completes, and the prefill queue is first come first served: the G/G/1 FIFO queue of the
+    Lindley recursion."""
+    rng = np.random.default_rng([16, seed])
+    n, c0 = 120, 5000
+    D = rng.integers(1, 12, n)
+    a = np.cumsum(rng.exponential(30000, n)).astype(np.int64)
+    wl = W.custom(a, np.ones(n, np.int32), D, dict(
+        max_batch=1, kv_blocks=1 << 20, c0_us=c0, c_prefill_tok_us=0, c_decode_seq_us=0, queue_cap=n),
+        W.make_replicas(1, policy=W.POLICY_SARATHI, guard=0, hysteresis_us=0))
+    tf, tl, _, _ = run_wl(wl).per_request()
+    C_prev = 0
+    for i in range(n):
+        start = max(int(a[i]), C_prev)
+        C_prev = start + int(D[i]) * c0
+        assert tl[0, i] == C_prev and tf[0, i] == start + c0
+
+
+def test_sarathi_decode_round_robin():
+    """"Round-robin ordering in the decode": the decode queue is ordered by the time of the request's last
+    token (tracked here from the per-iteration records), so whoever was left out of an iteration -- the KV pool is
+    small -- goes in front of those that were served in it; the prefill queue behind it is first come first served."""
+    wl = pressure_workload(2, n=140, kv_blocks=40, policy=W.POLICY_SARATHI, guard=0, delta=0, mean_gap_us=3000)
+    tr = wl.traces()
+    a = tr[0][0]
+    o = O.OracleSim(wl.sim, wl.replicas, tr)
+    t_last, d_seen = {}, {}
+    left_out_then_first = 0
+    prev_left, prev_served = set(), set()
+    for it in range(200000):
+        info, rows = o.step_replica(0)
+        if not info["executed"]:
+            break
+        started = [r for r in rows if r["klass"] == 0]
+        fresh = [r for r in rows if r["klass"] == 1]
+        assert [r["id"] for r in rows] == [r["id"] for r in started] + [r["id"] for r in fresh]      # decode-prioritised
+        assert all(d_seen.get(r["id"], 0) >= 1 for r in started) and all(d_seen.get(r["id"], 0) == 0 for r in fresh)
+        assert all(r["key"] == t_last[r["id"]] for r in started)                                    # round robin
+        assert all(r["key"] == int(a[r["id"]]) for r in fresh)                                      # FCFS prefill
+        assert [(r["key"], r["id"]) for r in started] == sorted((r["key"], r["id"]) for r in started)
+        assert [(r["key"], r["id"]) for r in fresh] == sorted((r["key"], r["id"]) for r in fresh)
+        pos = {r["id"]: j for j, r in enumerate(started)}
+        for x in prev_left:
+            for y in prev_served:
+                if x in pos and y in pos:
+                    assert pos[x] < pos[y]
+                    left_out_then_first += 1
+        prev_left = {r["id"] for r in started if r["want"] == 0}
+        prev_served = {r["id"] for r in started if r["want"] > 0 and r["d_after"] > d_seen.get(r["id"], 0)}
+        for r in rows:
+            if r["d_after"] > d_seen.get(r["id"], 0):
+                t_last[r["id"]] = info["t_end_us"]
+            d_seen[r["id"]] = r["d_after"]
+    assert left_out_then_first > 50 and o.stats()[0]["n_completed"] == 140
+
+
+@pytest.mark.parametrize("seed", range(3))
+def test_sarathi_is_distboost_without_boost_when_the_batch_cap_does_not_bind(seed):
+    """Decode first, chunked prefill piggy-backing first come first served: that is DistBoost (Eq. 3-6) with b_gamma = 0
+    (gamma = +inf) except for the order INSIDE the decode queue (round robin vs entry time), which only matters when
+    the batch cap, the token budget or the KV capacity cut the decode queue."""
+    wl_s = pressure_workload(seed, n=150, kv_blocks=1 << 16, policy=W.POLICY_SARATHI, guard=0, delta=0, max_batch=256,
+                             chunk_tokens=64, token_budget=1 << 15)
+    wl_d = pressure_workload(seed, n=150, kv_blocks=1 << 16, policy=W.POLICY_DISTBOOST, guard=0, delta=0, gamma=float("inf"),
+                             max_batch=256, chunk_tokens=64, token_budget=1 << 15)
+    s, d = run_wl(wl_s), run_wl(wl_d)
+    for x, y in zip(s.per_request(), d.per_request()):
+        assert np.array_equal(x, y)
+    assert s.stats()[0]["t_end_us"] == d.stats()[0]["t_end_us"]
