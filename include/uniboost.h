@@ -120,6 +120,15 @@ void ub_destroy(ub_sim*);
 int  ub_load_trace(ub_sim*, const int64_t* arrival_us, const int32_t* prompt_tok, const int32_t* decode_tok,
                    const uint32_t* n_req, int ptrs_on_device);
 
+/* Prefix / radix caching (A.5; rule M17 of DESIGN.md): as ub_load_trace plus hit_tok
+ * [n_traces][max_requests] (host or device like the others), the prompt tokens of each request already in the prefix
+ * cache, 0 <= h < P (else UB_EINVAL).  "Caching primarily reduces effective prefill work": the request prefills
+ * s_pre - h tokens, and its size signal is w~ = max(w, s_pre - h) with w the tokens processed so far -- the device
+ * record carries the effective prompt s_pre - h for both.  (The shared prefix's KV blocks belong to the cache and are
+ * not charged to the request's footprint.)  Synchronises. */
+int  ub_load_trace_prefix(ub_sim*, const int64_t* arrival_us, const int32_t* prompt_tok, const int32_t* decode_tok,
+                          const int32_t* hit_tok, const uint32_t* n_req, int ptrs_on_device);
+
 /* Set the replica table (host, [R]) and reset every replica to t = 0 with an empty queue.  Builds the
  * fixed-point boost table LUT[bin] = min(2^60, floor(b_gamma(k 2^bin tok_us 1e-6) 1e6 + 0.5)) us on the host
  * in fp64 (Eq. 2, rule M4) and uploads it.  Needs a loaded trace.  Synchronises. */

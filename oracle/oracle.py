@@ -70,6 +70,7 @@ def lib():
         L.orc_create.argtypes = [P(OrcConfig), P(C.c_void_p)]
         L.orc_destroy.argtypes = [C.c_void_p]; L.orc_destroy.restype = None
         L.orc_load_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_load_trace_prefix.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_set_replicas.argtypes = [C.c_void_p, P(OrcReplica)]
         L.orc_step.argtypes = [C.c_void_p, I64]
         L.orc_step_replica.argtypes = [C.c_void_p, I64, P(OrcStepInfo), P(OrcStepEntry)]
@@ -149,7 +150,7 @@ def _stats_to_dict(st):
 class OracleSim:
     """Drives the oracle from a workloads.Workload-like object (sim dict, replicas dict, traces())."""
 
-    def __init__(self, sim: dict, replicas: dict, traces):
+    def __init__(self, sim: dict, replicas: dict, traces, hits=None):
         L = lib()
         self.sim = dict(sim)
         cfg = OrcConfig(**{n: int(sim[n]) for n, _ in OrcConfig._fields_})
@@ -160,7 +161,12 @@ class OracleSim:
         a = np.ascontiguousarray(a, np.int64); p = np.ascontiguousarray(p, np.int32)
         d = np.ascontiguousarray(d, np.int32); n = np.ascontiguousarray(n, np.uint32)
         assert a.shape == (sim["n_traces"], sim["max_requests"])
-        _chk(L.orc_load_trace(h, a.ctypes.data, p.ctypes.data, d.ctypes.data, n.ctypes.data))
+        if hits is None:
+            _chk(L.orc_load_trace(h, a.ctypes.data, p.ctypes.data, d.ctypes.data, n.ctypes.data))
+        else:                                              # prefix-cache hit tokens per request (rule M17)
+            hh = np.ascontiguousarray(hits, np.int32)
+            assert hh.shape == a.shape
+            _chk(L.orc_load_trace_prefix(h, a.ctypes.data, p.ctypes.data, d.ctypes.data, hh.ctypes.data, n.ctypes.data))
         R = int(sim["n_replicas"])
         reps = (OrcReplica * R)()
         for r in range(R):

@@ -53,6 +53,7 @@ typedef struct {
 struct orc_sim {
   orc_config cfg;
   int64_t* arrival; int32_t* prompt; int32_t* decode; uint32_t* n_req;
+  int32_t* hit;        /* M17: prefix-cache hit tokens h_i per request (all 0 unless loaded with orc_load_trace_prefix) */
   int have_trace, have_reps;
   orc_rep* rep;
   orc_gamma_ada ada; int have_ada;
@@ -173,7 +174,7 @@ static void free_reps(orc_sim* s) {
 void orc_destroy(orc_sim* s) {
   if (!s) return;
   free_reps(s);
-  free(s->arrival); free(s->prompt); free(s->decode); free(s->n_req);
+  free(s->arrival); free(s->prompt); free(s->decode); free(s->n_req); free(s->hit);
   free(s);
 }
 
@@ -193,17 +194,34 @@ int orc_load_trace(orc_sim* s, const int64_t* a, const int32_t* p, const int32_t
     }
   }
   free_reps(s);
-  free(s->arrival); free(s->prompt); free(s->decode); free(s->n_req);
+  free(s->arrival); free(s->prompt); free(s->decode); free(s->n_req); free(s->hit);
+  s->hit = (int32_t*)calloc((size_t)(NT * N > 0 ? NT * N : 1), sizeof(int32_t));
   s->arrival = (int64_t*)malloc(sizeof(int64_t) * NT * N);
   s->prompt = (int32_t*)malloc(sizeof(int32_t) * NT * N);
   s->decode = (int32_t*)malloc(sizeof(int32_t) * NT * N);
   s->n_req = (uint32_t*)malloc(sizeof(uint32_t) * NT);
-  if (!s->arrival || !s->prompt || !s->decode || !s->n_req) return ORC_ENOMEM;
+  if (!s->arrival || !s->prompt || !s->decode || !s->n_req || !s->hit) return ORC_ENOMEM;
   memcpy(s->arrival, a, sizeof(int64_t) * NT * N);
   memcpy(s->prompt, p, sizeof(int32_t) * NT * N);
   memcpy(s->decode, d, sizeof(int32_t) * NT * N);
   memcpy(s->n_req, n_req, sizeof(uint32_t) * NT);
   s->have_trace = 1;
+  return ORC_OK;
+}
+
+/* M17 prefix / radix caching (A.5): a request with h_i cached prompt tokens needs only s_pre - h_i
+ * tokens of prefill ("caching primarily reduces effective prefill work") and its size signal becomes
+ * w~ = max(w, s_pre - h_i), w = the tokens processed so far.  hit: [n_traces][max_requests], 0 <= h < P. */
+int orc_load_trace_prefix(orc_sim* s, const int64_t* a, const int32_t* p, const int32_t* d, const int32_t* hit,
+                          const uint32_t* n_req) {
+  if (!hit) return ORC_EINVAL;
+  int rc = orc_load_trace(s, a, p, d, n_req);
+  if (rc) return rc;
+  const int64_t NT = s->cfg.n_traces, N = s->cfg.max_requests;
+  for (int64_t t = 0; t < NT; t++)
+    for (int64_t i = 0; i < (int64_t)n_req[t]; i++)
+      if (hit[t * N + i] < 0 || hit[t * N + i] >= p[t * N + i]) { s->have_trace = 0; return ORC_EINVAL; }
+  memcpy(s->hit, hit, sizeof(int32_t) * (size_t)(NT * N));
   return ORC_OK;
 }
 
@@ -380,6 +398,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
   const int64_t N = c->max_requests, tr = x->par.trace_id, nreq = s->n_req[tr];
   const int64_t* A = s->arrival + tr * N;
   const int32_t* Pp = s->prompt + tr * N;
+  const int32_t* Hh = s->hit + tr * N;     /* M17: prefix-cache hits; P below is the effective prefill work s_pre - h */
   const int32_t* Dd = s->decode + tr * N;
   const int64_t blk = c->block_tokens, B = c->kv_blocks;
   if (info) memset(info, 0, sizeof(*info));
@@ -403,8 +422,9 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
   for (int64_t j = 0; j < n; j++) {
     int64_t id = x->active[j];
     orc_req* q = &x->req[id];
-    int64_t P = Pp[id], D = Dd[id];
-    /* M3 SIGNAL: UNIFIED w~ = max(w, s_pre) with w = tokens processed => P + d;
+    int64_t P = Pp[id] - Hh[id], D = Dd[id];
+    /* M3 SIGNAL: UNIFIED w~ = max(w, s_pre) with w = tokens processed => P + d; with prefix-cache hits
+       w~ = max(w, s_pre - h) => (s_pre - h) + d, P being the effective prefill work here (M17);
        PHASE: prompt tokens in prefill else attained decode tokens */
     int64_t sig;
     if (x->par.signal_mode == ORC_SIG_UNIFIED) sig = P + q->d;
@@ -456,7 +476,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
   for (int64_t j = 0; j < n; j++) {
     if (cnt == c->max_batch || tok == c->token_budget) break;
     orc_req* q = &x->req[e[j].id];
-    int64_t P = Pp[e[j].id];
+    int64_t P = Pp[e[j].id] - Hh[e[j].id];
     if (!q->resident && newblocked) continue;
     int64_t rem = P + q->d - q->cached;                 /* tokens still to process before the next emission */
     int64_t want = c->chunk_tokens;                     /* KVNEED(r, c): next prefill chunk or decode step */
@@ -523,7 +543,7 @@ static int step_one(orc_sim* s, orc_rep* x, orc_step_info* info, orc_step_entry*
     int64_t id = e[j].id;
     orc_req* q = &x->req[id];
     q->resident = 1; q->swapped = 0; q->cached += (int32_t)e[j].want;
-    if (q->cached == Pp[id] + q->d) {
+    if (q->cached == Pp[id] - Hh[id] + q->d) {
       q->d++; x->tokens_emitted++;
       if (q->d == 1) { q->t_first = t_end; ev_add(&ev, EV_EMIT_FIRST, (uint32_t)id, 0); }
       else x->hist[orc_tbt_bin(t_end - q->t_last)]++;
@@ -761,7 +781,7 @@ int orc_class_percentiles(orc_sim* s, int64_t which, int64_t len_lo, int64_t len
     int64_t m = 0, tot = 0;
     for (int64_t i = 0; i < nreq; i++) {
       const orc_req* q = &x->req[i];
-      const int64_t len = (int64_t)s->prompt[tr * N + i] + (int64_t)s->decode[tr * N + i];
+      const int64_t len = (int64_t)s->prompt[tr * N + i] - (int64_t)s->hit[tr * N + i] + (int64_t)s->decode[tr * N + i];   /* (effective length, M17) */
       if (!q->completed || len < len_lo || len > len_hi) continue;
       const int64_t a = s->arrival[tr * N + i];
       v[m] = which == 0 ? q->t_first - a : (which == 1 ? q->t_last - a : q->t_preempt);

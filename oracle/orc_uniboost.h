@@ -136,6 +136,10 @@ void orc_destroy(orc_sim*);
 /* arrays are [n_traces][max_requests] row-major, arrival-sorted; n_req[n_traces] */
 int  orc_load_trace(orc_sim*, const int64_t* arrival_us, const int32_t* prompt_tok,
                     const int32_t* decode_tok, const uint32_t* n_req);
+/* Rule M17 (prefix / radix caching): as orc_load_trace plus hit[n_traces][max_requests] cached prompt
+ * tokens per request, 0 <= h < P: the request needs s_pre - h tokens of prefill and is signalled as w~ = max(w, s_pre - h). */
+int  orc_load_trace_prefix(orc_sim*, const int64_t* arrival_us, const int32_t* prompt_tok, const int32_t* decode_tok,
+                           const int32_t* hit_tok, const uint32_t* n_req);
 int  orc_set_replicas(orc_sim*, const orc_replica* reps);
 int  orc_step(orc_sim*, int64_t n_iters);                 /* every replica advances n_iters iterations */
 int  orc_step_replica(orc_sim*, int64_t replica, orc_step_info* info,

@@ -58,7 +58,7 @@ EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_st
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
            "ub_last_step_timing", "ub_set_iters_per_launch", "ub_set_gamma_ada", "ub_gamma_state", "ub_gamma_grid",
            "ub_percentile_curve", "ub_slo_attainment", "ub_debug_keys", "ub_debug_keys_stream", "ub_debug_set_state",
-           "ub_class_percentiles", "ub_preempt_time",
+           "ub_class_percentiles", "ub_preempt_time", "ub_load_trace_prefix",
            "ub_strerror")
 
 _lib = None
@@ -77,6 +77,7 @@ def lib():
         L.ub_create.argtypes = [P(UbConfig), P(vp)]
         L.ub_destroy.argtypes = [vp]; L.ub_destroy.restype = None
         L.ub_load_trace.argtypes = [vp, vp, vp, vp, vp, C.c_int]
+        L.ub_load_trace_prefix.argtypes = [vp, vp, vp, vp, vp, vp, C.c_int]
         L.ub_set_replicas.argtypes = [vp, P(UbReplica)]
         L.ub_step.argtypes = [vp, U32, P(U64)]
         L.ub_run.argtypes = [vp, U64, P(U64)]
@@ -135,6 +136,14 @@ def ub_load_trace(h, arrival_us, prompt_tok, decode_tok, n_req, ptrs_on_device=F
     a = np.ascontiguousarray(arrival_us, np.int64); p = np.ascontiguousarray(prompt_tok, np.int32)
     d = np.ascontiguousarray(decode_tok, np.int32); n = np.ascontiguousarray(n_req, np.uint32)
     return _chk(lib().ub_load_trace(h, a.ctypes.data, p.ctypes.data, d.ctypes.data, n.ctypes.data, 0))
+
+
+def ub_load_trace_prefix(h, arrival_us, prompt_tok, decode_tok, hit_tok, n_req):
+    """As ub_load_trace (host numpy arrays) plus the prefix-cache hit tokens per request (rule M17)."""
+    a = np.ascontiguousarray(arrival_us, np.int64); p = np.ascontiguousarray(prompt_tok, np.int32)
+    d = np.ascontiguousarray(decode_tok, np.int32); hh = np.ascontiguousarray(hit_tok, np.int32)
+    n = np.ascontiguousarray(n_req, np.uint32)
+    return _chk(lib().ub_load_trace_prefix(h, a.ctypes.data, p.ctypes.data, d.ctypes.data, hh.ctypes.data, n.ctypes.data, 0))
 
 
 def ub_set_replicas(h, reps):
@@ -221,7 +230,7 @@ class Sim:
     """Drives libuniboost.so from a workloads.Workload-like description (sim dict, replica table, traces)."""
 
     def __init__(self, sim: dict, replicas: dict, traces, iters_per_launch: int = 1, device: int = 0,
-                 stream: int | None = None):
+                 stream: int | None = None, hits=None):
         import torch  # plumbing only: the current CUDA stream
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2606_18431_b200 needs a CUDA device (B200, sm_100a); there is no CPU fallback")
@@ -233,7 +242,10 @@ class Sim:
         self._h = ub_create(make_config(sim, iters_per_launch, device, stream))
         a, p, d, n = traces
         assert np.shape(a) == (sim["n_traces"], sim["max_requests"])
-        ub_load_trace(self._h, a, p, d, n)
+        if hits is None:
+            ub_load_trace(self._h, a, p, d, n)
+        else:
+            ub_load_trace_prefix(self._h, a, p, d, hits, n)
         ub_set_replicas(self._h, make_replicas(replicas, self.R))
 
     @classmethod

@@ -155,8 +155,8 @@ void ub_destroy(ub_sim* s) {
   delete s;
 }
 
-int ub_load_trace(ub_sim* s, const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
-                  int on_device) {
+static int load_trace_impl(ub_sim* s, const int64_t* a, const int32_t* p, const int32_t* d, const int32_t* hit,
+                           const uint32_t* n_req, int on_device) {
   if (!s || !a || !p || !d || !n_req) return UB_EINVAL;
   if (set_dev(s)) return UB_ECUDA;
   const size_t NT = s->cfg.n_traces, N = s->cfg.max_requests, tot = NT * N;
@@ -167,28 +167,29 @@ int ub_load_trace(ub_sim* s, const int64_t* a, const int32_t* p, const int32_t* 
   s->have_trace = false; s->have_reps = false;
   if (!s->d_TR) { int rc = dmalloc(&s->d_TR, tot); if (rc) return rc; }
   CK(cudaMemcpyAsync(s->d_nreq, s->h_nreq.data(), NT * 4, cudaMemcpyHostToDevice, s->stream));
-  int64_t* da = nullptr; int32_t* dp = nullptr; int32_t* dd = nullptr;
-  const int64_t* ua = a; const int32_t* up = p; const int32_t* ud = d;
+  int64_t* da = nullptr; int32_t* dp = nullptr; int32_t* dd = nullptr; int32_t* dh = nullptr;
+  const int64_t* ua = a; const int32_t* up = p; const int32_t* ud = d; const int32_t* uh = hit;
   int rc = UB_OK;
   if (!on_device) {
-    if ((rc = dmalloc(&da, tot)) || (rc = dmalloc(&dp, tot)) || (rc = dmalloc(&dd, tot))) {
-      cudaFree(da); cudaFree(dp); cudaFree(dd); return rc;
+    if ((rc = dmalloc(&da, tot)) || (rc = dmalloc(&dp, tot)) || (rc = dmalloc(&dd, tot)) || (hit && (rc = dmalloc(&dh, tot)))) {
+      cudaFree(da); cudaFree(dp); cudaFree(dd); cudaFree(dh); return rc;
     }
     if (cudaMemcpyAsync(da, a, tot * 8, cudaMemcpyHostToDevice, s->stream) != cudaSuccess ||
         cudaMemcpyAsync(dp, p, tot * 4, cudaMemcpyHostToDevice, s->stream) != cudaSuccess ||
-        cudaMemcpyAsync(dd, d, tot * 4, cudaMemcpyHostToDevice, s->stream) != cudaSuccess) {
-      cudaGetLastError(); cudaFree(da); cudaFree(dp); cudaFree(dd); return UB_ECUDA;
+        cudaMemcpyAsync(dd, d, tot * 4, cudaMemcpyHostToDevice, s->stream) != cudaSuccess ||
+        (hit && cudaMemcpyAsync(dh, hit, tot * 4, cudaMemcpyHostToDevice, s->stream) != cudaSuccess)) {
+      cudaGetLastError(); cudaFree(da); cudaFree(dp); cudaFree(dd); cudaFree(dh); return UB_ECUDA;
     }
-    ua = da; up = dp; ud = dd;
+    ua = da; up = dp; ud = dd; uh = hit ? dh : nullptr;
   }
   s->h_word[0] = ~0ull;
   cudaMemcpyAsync(s->d_word, s->h_word, 8, cudaMemcpyHostToDevice, s->stream);
-  launch_pack_validate(ua, up, ud, s->d_nreq, (uint32_t)NT, (uint32_t)N, s->cfg.kv_blocks, s->cfg.block_tokens,
+  launch_pack_validate(ua, up, ud, uh, s->d_nreq, (uint32_t)NT, (uint32_t)N, s->cfg.kv_blocks, s->cfg.block_tokens,
                        s->d_TR, reinterpret_cast<int*>(s->d_word), s->stream);
   cudaMemcpyAsync(s->h_word, s->d_word, 8, cudaMemcpyDeviceToHost, s->stream);
   cudaError_t e = cudaStreamSynchronize(s->stream);
   if (e == cudaSuccess) e = cudaGetLastError();
-  cudaFree(da); cudaFree(dp); cudaFree(dd);
+  cudaFree(da); cudaFree(dp); cudaFree(dd); cudaFree(dh);
   if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
   if (s->h_word[0] != ~0ull) {
     const int kind = (int)(s->h_word[0] & 3ull);
@@ -197,6 +198,15 @@ int ub_load_trace(ub_sim* s, const int64_t* a, const int32_t* p, const int32_t* 
   s->dev.TR = s->d_TR;
   s->have_trace = true;
   return UB_OK;
+}
+
+int ub_load_trace(ub_sim* s, const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req, int on_device) {
+  return load_trace_impl(s, a, p, d, nullptr, n_req, on_device);
+}
+int ub_load_trace_prefix(ub_sim* s, const int64_t* a, const int32_t* p, const int32_t* d, const int32_t* hit,
+                         const uint32_t* n_req, int on_device) {
+  if (!hit) return UB_EINVAL;
+  return load_trace_impl(s, a, p, d, hit, n_req, on_device);
 }
 
 // Eq. 2 / BOOST in fixed point, rule M4:

@@ -7,33 +7,37 @@ namespace ub {
 // ------------------------------------------------------------------ trace validation + packing (ub_load_trace)
 // err: first offending (trace, request) in row-major scan order, encoded (linear index << 2 | kind),
 // kind 0 = arrival outside [0, 2^61] (UB_EINVAL), 1 = arrivals decrease (UB_EUNSORTED), 2 = infeasible request.
+// hit (nullable): prefix-cache hit tokens per request (rule M17): the record carries the effective
+// prefill work s_pre - h, which is also what the size signal w~ = max(w, s_pre - h) starts from.
 __global__ void k_pack_validate(const int64_t* __restrict__ a, const int32_t* __restrict__ p,
-                                const int32_t* __restrict__ d, const uint32_t* __restrict__ n_req,
+                                const int32_t* __restrict__ d, const int32_t* __restrict__ hit,
+                                const uint32_t* __restrict__ n_req,
                                 uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* __restrict__ out,
                                 unsigned long long* err) {
   const size_t total = (size_t)NT * N;
   for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < total; g += (size_t)gridDim.x * blockDim.x) {
     const uint32_t tr = (uint32_t)(g / N), i = (uint32_t)(g % N);
-    Rec0 rec; rec.a = a[g]; rec.P = (uint32_t)p[g]; rec.D = (uint32_t)d[g];
+    const int64_t h = hit ? (int64_t)hit[g] : 0;
+    Rec0 rec; rec.a = a[g]; rec.P = (uint32_t)((int64_t)p[g] - h); rec.D = (uint32_t)d[g];
     out[g] = rec;
     if (i >= n_req[tr]) continue;
     const int64_t ai = rec.a;
     const int64_t P = p[g], D = d[g];
     int kind = -1;
-    if (ai < 0 || ai > ((int64_t)1 << 61)) kind = 0;
+    if (ai < 0 || ai > ((int64_t)1 << 61) || h < 0 || (P >= 1 && h >= P)) kind = 0;
     else if (i > 0 && ai < a[g - 1]) kind = 1;
     else if (P < 1 || D < 1 || (P + D + blk - 1) / blk > (int64_t)B) kind = 2;
     if (kind >= 0) atomicMin(err, ((unsigned long long)g << 2) | (unsigned long long)kind);
   }
 }
 
-void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
+void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const int32_t* hit, const uint32_t* n_req,
                           uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st) {
   const size_t total = (size_t)NT * N;
   int blocks = (int)((total + 255) / 256);
   if (blocks > 148 * 16) blocks = 148 * 16;
   if (blocks < 1) blocks = 1;
-  k_pack_validate<<<blocks, 256, 0, st>>>(a, p, d, n_req, NT, N, B, blk, out,
+  k_pack_validate<<<blocks, 256, 0, st>>>(a, p, d, hit, n_req, NT, N, B, blk, out,
                                           reinterpret_cast<unsigned long long*>(err));
 }
 

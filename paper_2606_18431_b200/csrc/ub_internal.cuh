@@ -106,7 +106,7 @@ void launch_debug_keys_stream(const SimDev& s, uint32_t r, uint32_t n, uint32_t*
 void launch_gamma_ada(const SimDev& s, uint32_t rbeg, uint32_t rend, cudaStream_t st);   // ub_aux.cu
 void launch_ada_init(const SimDev& s, cudaStream_t st);
 int  step_configure(uint32_t Q);
-void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const uint32_t* n_req,
+void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, const int32_t* hit, const uint32_t* n_req,
                           uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st);
 void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st);
 void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* live, cudaStream_t st);
