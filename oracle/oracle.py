@@ -89,6 +89,7 @@ def lib():
         L.orc_percentile_curve.argtypes = [C.c_void_p, I64, C.c_void_p, I64, C.c_void_p]
         L.orc_slo_attainment.argtypes = [C.c_void_p, I64, C.c_void_p, I64, C.c_void_p]
         L.orc_preempt_time.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_jsq_run.argtypes = [C.c_void_p, I64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, I64, C.c_void_p]
         L.orc_class_percentiles.argtypes = [C.c_void_p, I64, I64, I64, C.c_void_p, I64, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_set_gamma_ada.argtypes = [C.c_void_p, P(OrcGammaAda), C.c_void_p]
         L.orc_gamma_state.argtypes = [C.c_void_p, I64, P(I64), P(I64), P(I64)]
@@ -180,6 +181,17 @@ class OracleSim:
         pm = np.ascontiguousarray(permille, np.int64)
         out = np.zeros((self.R, len(pm)), np.int64)
         _chk(lib().orc_percentile_curve(self._h, int(which), pm.ctypes.data, len(pm), out.ctypes.data))
+        return out
+
+    def jsq_run(self, cluster_size, arrival_us, prompt_tok, decode_tok, n_arr):
+        """Rule M18: route the [C][NA] global streams over clusters of `cluster_size` replicas by join-the-shortest-queue
+        and run everything to completion; returns assign [C][NA] (replica number within the cluster, -1 = no arrival)."""
+        a = np.ascontiguousarray(arrival_us, np.int64); p = np.ascontiguousarray(prompt_tok, np.int32)
+        d = np.ascontiguousarray(decode_tok, np.int32); n = np.ascontiguousarray(n_arr, np.uint32)
+        assert a.ndim == 2 and a.shape == p.shape == d.shape and n.shape == (a.shape[0],)
+        out = np.full(a.shape, -1, np.int32)
+        _chk(lib().orc_jsq_run(self._h, int(cluster_size), a.ctypes.data, p.ctypes.data, d.ctypes.data, n.ctypes.data,
+                               a.shape[1], out.ctypes.data))
         return out
 
     def preempt_time(self):

@@ -246,11 +246,11 @@ int orc_set_replicas(orc_sim* s, const orc_replica* reps) {
     orc_rep* x = &s->rep[r];
     x->par = reps[r];
     int64_t tr = x->par.trace_id, n = s->n_req[tr];
-    x->req = (orc_req*)calloc((size_t)(n > 0 ? n : 1), sizeof(orc_req));
+    x->req = (orc_req*)calloc((size_t)(N > 0 ? N : 1), sizeof(orc_req));   /* (row length: a JSQ router appends, M18) */
     x->active = (int32_t*)calloc((size_t)c->queue_cap, sizeof(int32_t));
     x->hist = (uint32_t*)calloc(TBT_BINS, sizeof(uint32_t));
     if (!x->req || !x->active || !x->hist) return ORC_ENOMEM;
-    for (int64_t i = 0; i < n; i++) { x->req[i].t_first = -1; x->req[i].t_last = -1; x->req[i].lockbin = -1; x->req[i].preempt_since = -1; }
+    for (int64_t i = 0; i < N; i++) { x->req[i].t_first = -1; x->req[i].t_last = -1; x->req[i].lockbin = -1; x->req[i].preempt_since = -1; }
     /* boost table (M4): one entry per bin; EXACT quantiser => one entry per signal value */
     int64_t nb = LUT_CAP_GEOM;
     if (x->par.quant_mode == ORC_Q_EXACT) {
@@ -641,6 +641,63 @@ int orc_run(orc_sim* s, int64_t max_iters, int64_t* iters_done) {
   }
   if (iters_done) *iters_done = mx;
   return live ? ORC_ELIVELOCK : ORC_OK;
+}
+
+/* ---------- M18: a cluster of replicas behind a join-the-shortest-queue router (Table 9) ----------
+ * "Cluster-level routers decide which instance a request is sent to; UniBoost decides how to schedule requests within
+ * that instance."  Replicas c K .. c K + K - 1 form cluster c and start with empty traces; the cluster's arrivals come in
+ * one global stream.  An arrival at time a goes to the replica with the fewest requests in the system at time a --
+ * assigned to it and not completed by a (completion time t_last <= a counts as gone) --, the lowest replica number on
+ * a tie.  A replica's state at time a is the result of every iteration that STARTS before a (an iteration that starts at
+ * a would already ingest the arrival). */
+static int64_t jsq_next_start(const orc_sim* s, const orc_rep* x) {
+  if (x->n_active > 0) return x->t;
+  const int64_t tr = x->par.trace_id;
+  if (x->next >= (int64_t)s->n_req[tr]) return INT64_MAX;                  /* nothing to do */
+  const int64_t a = s->arrival[tr * s->cfg.max_requests + x->next];
+  return a > x->t ? a : x->t;                                              /* idle jump (M6) */
+}
+
+int orc_jsq_run(orc_sim* s, int64_t K, const int64_t* arrival, const int32_t* prompt, const int32_t* decode,
+                const uint32_t* n_arr, int64_t NA, int32_t* assign) {
+  if (!s || !arrival || !prompt || !decode || !n_arr || K < 1 || NA < 0) return ORC_EINVAL;
+  if (!s->have_reps) return ORC_ESTATE;
+  const orc_config* c = &s->cfg;
+  const int64_t R = c->n_replicas, N = c->max_requests;
+  if (R % K != 0 || c->n_traces != R) return ORC_EINVAL;
+  const int64_t C = R / K;
+  for (int64_t r = 0; r < R; r++)
+    if (s->rep[r].par.trace_id != r || s->n_req[r] != 0 || s->rep[r].iterations != 0 || s->rep[r].ada) return ORC_ESTATE;
+  for (int64_t cl = 0; cl < C; cl++) {
+    if ((int64_t)n_arr[cl] > NA) return ORC_EINVAL;
+    for (int64_t j = 0; j < (int64_t)n_arr[cl]; j++) {
+      const int64_t a = arrival[cl * NA + j], P = prompt[cl * NA + j], D = decode[cl * NA + j];
+      if (a < 0 || a > ((int64_t)1 << 61)) return ORC_EINVAL;
+      if (j > 0 && a < arrival[cl * NA + j - 1]) return ORC_EUNSORTED;
+      if (P < 1 || D < 1 || (P + D + c->block_tokens - 1) / c->block_tokens > c->kv_blocks) return ORC_EINFEASIBLE;
+    }
+  }
+  for (int64_t cl = 0; cl < C; cl++) {
+    for (int64_t j = 0; j < (int64_t)n_arr[cl]; j++) {
+      const int64_t a = arrival[cl * NA + j];
+      int64_t best = -1, best_n = 0;
+      for (int64_t k = 0; k < K; k++) {
+        orc_rep* x = &s->rep[cl * K + k];
+        while (jsq_next_start(s, x) < a) { int rc = step_one(s, x, NULL, NULL); if (rc < 0) return rc; }
+        int64_t in_system = 0;                                             /* assigned and not completed by time a */
+        for (int64_t i = 0; i < (int64_t)s->n_req[cl * K + k]; i++)
+          if (!(x->req[i].completed && x->req[i].t_last <= a)) in_system++;
+        if (best < 0 || in_system < best_n) { best = k; best_n = in_system; }
+      }
+      const int64_t tr = cl * K + best;
+      if ((int64_t)s->n_req[tr] >= N) return ORC_EINVAL;                   /* the replica's row is full */
+      const int64_t at = tr * N + s->n_req[tr];
+      s->arrival[at] = a; s->prompt[at] = prompt[cl * NA + j]; s->decode[at] = decode[cl * NA + j];
+      s->n_req[tr]++;
+      if (assign) assign[cl * NA + j] = (int32_t)best;
+    }
+  }
+  return orc_run(s, INT64_MAX, NULL);                                      /* every replica serves what it got */
 }
 
 /* ---------- read-out ---------- */

@@ -164,6 +164,13 @@ int  orc_preempt_time(orc_sim*, int64_t* out);
  * preemption time (2) -> out [R][n]; their number -> count [R] (nullable); their sum -> sum [R] (nullable). */
 int  orc_class_percentiles(orc_sim*, int64_t which, int64_t len_lo, int64_t len_hi, const int64_t* permille, int64_t n,
                            int64_t* out, int64_t* count, int64_t* sum);
+/* Rule M18: clusters of K replicas behind a join-the-shortest-queue router (Table 9).
+ * The simulator must hold n_replicas = C K replicas, replica r on its own trace r, all traces empty, no iteration run.
+ * arrival / prompt / decode: [C][NA] global streams (arrival-sorted per cluster), n_arr[C] their lengths.  Every arrival
+ * goes to the replica of its cluster with the fewest requests in the system at its arrival time (lowest number on a
+ * tie); then every replica runs to completion.  assign (nullable): [C][NA] replica number within the cluster. */
+int  orc_jsq_run(orc_sim*, int64_t cluster_size, const int64_t* arrival_us, const int32_t* prompt_tok,
+                 const int32_t* decode_tok, const uint32_t* n_arr, int64_t max_arrivals, int32_t* assign);
 int  orc_boost_lut(orc_sim*, int64_t replica, int64_t* lut /* [cap] */, int64_t cap, int64_t* nb);
 int  orc_tbt_hist(orc_sim*, int64_t replica, uint32_t* hist /* [4352] */);
 /* stand-alone helpers exposed so the pins can hit them directly */
