@@ -240,6 +240,21 @@ int  ub_class_percentiles(ub_sim*, uint32_t which, uint32_t len_lo, uint32_t len
  * Synchronises. */
 int  ub_preempt_time(ub_sim*, int64_t* t_preempt_us, int on_device);
 
+/* Clusters of replicas behind a join-the-shortest-queue router ("Composability with Global
+ * Dispatch Policies", Table 9; rule M18 of DESIGN.md).  The handle must hold n_replicas =
+ * n_clusters x cluster_size replicas (cluster_size <= 32), replica r on its own trace r, every trace loaded EMPTY
+ * (n_req = 0; max_requests is the room of a replica's row), replicas set and no iteration run; gamma-Ada off.
+ * arrival_us / prompt_tok / decode_tok: host, [n_clusters][max_arrivals], one global stream per cluster, arrival-sorted;
+ * n_arrivals: host [n_clusters].  Arrival by arrival, every replica of the cluster executes the iterations that START
+ * before the arrival time (a time-fenced run of the step kernels); then the arrival joins the replica with the fewest
+ * requests in the system at that instant -- assigned to it and not completed by then --, the lowest replica number on a
+ * tie (one warp per cluster: a min-reduction over the cluster's replicas), and is appended to that replica's trace.
+ * After the last arrival every replica runs to completion (ub_run).  assign (host, nullable): [n_clusters][max_arrivals],
+ * the replica number within the cluster each arrival joined (-1 = no arrival).  Errors as ub_load_trace for the streams;
+ * UB_EINVAL if a replica's row overflows; UB_ESTATE on a handle that is not in the state above.  Synchronises. */
+int  ub_jsq_run(ub_sim*, uint32_t cluster_size, uint32_t n_clusters, uint32_t max_arrivals, const int64_t* arrival_us,
+                const int32_t* prompt_tok, const int32_t* decode_tok, const uint32_t* n_arrivals, int32_t* assign);
+
 /* gamma-Ada (Eq. 9, UPDATEGAMMA PAPER.md:588-601; rule M13 of DESIGN.md),
  * integer-only so that schedules stay bit-exact.  gamma is kept as gamma_u = gamma * 1e6.  At the start of an executed
  * iteration of an adaptive replica, if a request completed since the last update and >= min_samples have completed:

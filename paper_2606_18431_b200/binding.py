@@ -58,7 +58,7 @@ EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_st
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
            "ub_last_step_timing", "ub_set_iters_per_launch", "ub_set_gamma_ada", "ub_gamma_state", "ub_gamma_grid",
            "ub_percentile_curve", "ub_slo_attainment", "ub_debug_keys", "ub_debug_keys_stream", "ub_debug_set_state",
-           "ub_class_percentiles", "ub_preempt_time", "ub_load_trace_prefix",
+           "ub_class_percentiles", "ub_preempt_time", "ub_load_trace_prefix", "ub_jsq_run",
            "ub_strerror")
 
 _lib = None
@@ -96,6 +96,7 @@ def lib():
         L.ub_slo_attainment.argtypes = [vp, U32, vp, U32, vp]
         L.ub_class_percentiles.argtypes = [vp, U32, U32, U32, vp, U32, vp, vp, vp]
         L.ub_preempt_time.argtypes = [vp, vp, C.c_int]
+        L.ub_jsq_run.argtypes = [vp, U32, U32, U32, vp, vp, vp, vp, vp]
         L.ub_set_gamma_ada.argtypes = [vp, P(UbGammaAda), vp]
         L.ub_gamma_state.argtypes = [vp, U32, P(I64), P(C.c_int32), P(U64)]
         L.ub_gamma_grid.argtypes = [vp, vp]
@@ -310,6 +311,17 @@ class Sim:
         _chk(lib().ub_class_percentiles(self._h, int(which), int(len_lo), hi, pm.ctypes.data, len(pm), out.ctypes.data,
                                         cnt.ctypes.data, tot.ctypes.data))
         return out, cnt.astype(np.int64), tot
+
+    def jsq_run(self, cluster_size, arrival_us, prompt_tok, decode_tok, n_arr):
+        """ub_jsq_run: route the [C][NA] global streams over clusters of `cluster_size` replicas by join-the-shortest-queue
+        and run everything to completion; returns assign [C][NA] (replica number within the cluster, -1 = no arrival)."""
+        a = np.ascontiguousarray(arrival_us, np.int64); p = np.ascontiguousarray(prompt_tok, np.int32)
+        d = np.ascontiguousarray(decode_tok, np.int32); n = np.ascontiguousarray(n_arr, np.uint32)
+        assert a.ndim == 2 and a.shape == p.shape == d.shape and n.shape == (a.shape[0],)
+        out = np.full(a.shape, -1, np.int32)
+        _chk(lib().ub_jsq_run(self._h, int(cluster_size), a.shape[0], a.shape[1], a.ctypes.data, p.ctypes.data,
+                              d.ctypes.data, n.ctypes.data, out.ctypes.data))
+        return out
 
     def preempt_time(self):
         """[R][N] int64 microseconds each request spent preempted (rule M15)."""

@@ -337,9 +337,13 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
 // A round = one launch_step over all replicas.  With many replicas it is issued as nsplit parts on as many streams
 // (the caller's and internal ones, fork / join by events): replicas are independent, so while the last warps of one
 // part finish, the other parts' CTAs already fill the freed SMs.
-static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
+// tlimit (device, [R], nullable): a fenced run (JSQ router, rule M18) -- one launch in which every replica executes the
+// iterations that start before its limit.
+static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches, const int64_t* tlimit = nullptr) {
   const bool ada = s->d_ada_ring != nullptr;         // UPDATEGAMMA opens every iteration: one iteration per launch
-  const uint32_t ipl = (!ada && s->cfg.iters_per_launch > 1) ? s->cfg.iters_per_launch : 1;
+  constexpr uint32_t kFenced = 1u << 20;             // iterations a fenced launch may run (the fence ends it long before)
+  if (tlimit) n_iters = kFenced;
+  const uint32_t ipl = tlimit ? kFenced : ((!ada && s->cfg.iters_per_launch > 1) ? s->cfg.iters_per_launch : 1);
   const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
   const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
   // the drift group (SRPT / LAS replicas) is one more independent set of replicas: its launches go to a stream of their
@@ -361,18 +365,18 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
       const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
       if (ada) launch_gamma_ada(s->dev, rb, re, i ? s->aux[i - 1] : s->stream);
       launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, s->round_no,
-                  lst ? s->d_live + rb : nullptr, lst ? s->livecnt[i] : 0u, false, i ? s->aux[i - 1] : s->stream);
+                  lst ? s->d_live + rb : nullptr, lst ? s->livecnt[i] : 0u, false, tlimit, i ? s->aux[i - 1] : s->stream);
     }
-    if (nd) launch_step(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, k, 0, nd, s->round_no, dlist, nd, true, dst);
+    if (nd) launch_step(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, k, 0, nd, s->round_no, dlist, nd, true, tlimit, dst);
     n_iters -= k; nl++; s->round_no++;
     // what k_stream queued for the team kernels runs at the end of the call (all owed iterations at once); with
     // gamma-Ada after every round, because UPDATEGAMMA sits between the iterations
     if (ada || n_iters == 0) {
       for (uint32_t i = 0; i < ns; i++) {
         const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
-        flush_slow(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, rb, re, i ? s->aux[i - 1] : s->stream);
+        flush_slow(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, rb, re, tlimit, i ? s->aux[i - 1] : s->stream);
       }
-      if (nd) flush_slow(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, 0, nd, dst);
+      if (nd) flush_slow(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, 0, nd, tlimit, dst);
     }
   }
   if (ns > 1 || nd) {
@@ -939,4 +943,73 @@ int ub_debug_set_state(ub_sim* s, uint32_t r, uint32_t n, const uint32_t* id, co
   cudaFree(dv);
   if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
   return herr == 0 ? UB_OK : (herr == 2 ? UB_ESTATE : UB_EINVAL);
+}
+
+// ---------------------------------------------------------------------------------------------- JSQ router (rule M18)
+int ub_jsq_run(ub_sim* s, uint32_t K, uint32_t C, uint32_t NA, const int64_t* a, const int32_t* p, const int32_t* d,
+               const uint32_t* n_arr, int32_t* assign) {
+  if (!s || !a || !p || !d || !n_arr || K < 1 || K > 32 || C < 1) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  const ub_config& c = s->cfg;
+  if ((uint64_t)K * C != c.n_replicas || c.n_traces != c.n_replicas || c.max_requests >= (1u << 26)) return UB_EINVAL;
+  if (s->d_ada_ring) return UB_ESTATE;                             // (gamma-Ada runs one iteration per launch: no fenced runs)
+  if (set_dev(s)) return UB_ECUDA;
+  const size_t R = c.n_replicas;
+  for (size_t r = 0; r < R; r++) if (s->h_reps[r].trace_id != r || s->h_nreq[r] != 0) return UB_ESTATE;
+  {
+    std::vector<Hdr> hd(R);
+    CK(cudaMemcpyAsync(hd.data(), s->d_hdr, R * sizeof(Hdr), cudaMemcpyDeviceToHost, s->stream));
+    CK(cudaStreamSynchronize(s->stream));
+    for (size_t r = 0; r < R; r++) if (hd[r].iterations != 0) return UB_ESTATE;
+  }
+  uint32_t maxn = 0;
+  for (uint32_t cl = 0; cl < C; cl++) {                            // the same checks ub_load_trace makes on a trace
+    if (n_arr[cl] > NA) return UB_EINVAL;
+    if (n_arr[cl] > maxn) maxn = n_arr[cl];
+    for (uint32_t j = 0; j < n_arr[cl]; j++) {
+      const int64_t aj = a[(size_t)cl * NA + j], P = p[(size_t)cl * NA + j], D = d[(size_t)cl * NA + j];
+      if (aj < 0 || aj > ((int64_t)1 << 61)) return UB_EINVAL;
+      if (j > 0 && aj < a[(size_t)cl * NA + j - 1]) return UB_EUNSORTED;
+      if (P < 1 || D < 1 || (P + D + c.block_tokens - 1) / c.block_tokens > (int64_t)c.kv_blocks) return UB_EINFEASIBLE;
+    }
+  }
+  const size_t tot = (size_t)C * NA;
+  int64_t* da = nullptr; int32_t* dp = nullptr; int32_t* dd = nullptr; uint32_t* dn = nullptr;
+  int64_t* dl = nullptr; int32_t* das = nullptr; int* derr = nullptr;
+  int rc = UB_OK;
+  auto cleanup = [&]() { cudaFree(da); cudaFree(dp); cudaFree(dd); cudaFree(dn); cudaFree(dl); cudaFree(das); cudaFree(derr); };
+  if ((rc = dmalloc(&da, tot)) || (rc = dmalloc(&dp, tot)) || (rc = dmalloc(&dd, tot)) || (rc = dmalloc(&dn, (size_t)C)) ||
+      (rc = dmalloc(&dl, R)) || (rc = dmalloc(&das, tot)) || (rc = dmalloc(&derr, 1))) { cleanup(); return rc; }
+  cudaError_t e = cudaSuccess;
+  if (tot) {
+    e = cudaMemcpyAsync(da, a, tot * 8, cudaMemcpyHostToDevice, s->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dp, p, tot * 4, cudaMemcpyHostToDevice, s->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dd, d, tot * 4, cudaMemcpyHostToDevice, s->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(das, 0xFF, tot * 4, s->stream);      // -1 = no arrival
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(dn, n_arr, (size_t)C * 4, cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(derr, 0, sizeof(int), s->stream);
+  if (e != cudaSuccess) { cudaGetLastError(); cleanup(); return UB_ECUDA; }
+  JsqArgs J; J.K = K; J.C = C; J.NA = NA; J.a = da; J.p = dp; J.d = dd; J.n_arr = dn; J.tlimit = dl; J.assign = das;
+  J.count = s->d_count; J.err = derr;
+  // arrival by arrival: [route arrival j - 1, move the fences to arrival j] -> [every replica runs the iterations that
+  // start before its fence]; clusters are the batch dimension
+  s->use_list = false;
+  for (int64_t j = 0; j <= (int64_t)maxn && rc == UB_OK; j++) {
+    launch_jsq_dispatch(s->dev, J, j - 1, s->stream);
+    if (j < (int64_t)maxn) { uint32_t nl = 0; rc = issue_steps(s, 0, &nl, dl); }
+  }
+  int herr = 0;
+  if (rc == UB_OK) {
+    e = cudaMemcpyAsync(&herr, derr, sizeof(int), cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess && assign && tot) e = cudaMemcpyAsync(assign, das, tot * 4, cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s->h_nreq.data(), s->d_nreq, R * 4, cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) { cudaGetLastError(); rc = UB_ECUDA; }
+  }
+  cleanup();
+  if (rc) return rc;
+  if (herr) return UB_EINVAL;                                       // some replica's trace row (max_requests) was too short
+  return ub_run(s, ~0ull >> 1, nullptr);                            // every replica serves what it got
 }

@@ -162,6 +162,50 @@ void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, const ui
   if (rend > rbeg) k_compact_live<<<148, 256, 0, st>>>(s, rbeg, rend, in, drift_group ? 1u : 0u, out, cnt);
 }
 
+// ------------------------------------------------------------------ JSQ router (rule M18; Table 9)
+// One warp per cluster of K <= 32 replicas (lane k = replica c K + k).  Called between two fenced runs: every replica of
+// the cluster has executed every iteration that starts before arrival j of its cluster's stream.  The arrival goes to
+// the replica with the fewest requests in the system at that instant -- assigned to it and not completed by then: the
+// completions of the replica's last iteration count only if that iteration has ended by the arrival time --, lowest
+// replica number on a tie; it is appended to that replica's trace.  Then the fence of the cluster moves to arrival j + 1
+// (INT64_MIN when the stream is exhausted: the replicas wait for the final free run).  j = -1: only the first fence.
+__global__ void k_jsq_dispatch(SimDev s, JsqArgs J, long long j) {
+  const uint32_t c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), k = threadIdx.x & 31u;
+  if (c >= J.C) return;
+  const uint32_t na = J.n_arr[c];
+  if (j >= 0 && (uint64_t)j < na) {
+    const int64_t a = J.a[(size_t)c * J.NA + j];
+    const uint32_t r = c * J.K + k;
+    uint32_t load = 0xFFFFFFFFu;
+    Hdr* h = nullptr;
+    uint32_t* nreq = const_cast<uint32_t*>(s.n_req);
+    if (k < J.K) {
+      h = s.hdr + r;
+      const uint32_t gone = h->n_completed - ((h->t > a) ? h->last_done : 0u);
+      load = nreq[r] - gone;
+    }
+    const uint32_t best = __reduce_min_sync(0xffffffffu, load >= (1u << 26) ? 0xFFFFFFFFu : ((load << 5) | k));
+    if (k == (best & 31u) && k < J.K) {
+      const uint32_t at = nreq[r];
+      if (at >= s.N) atomicExch(J.err, 1);                          // the replica's row is full
+      else {
+        Rec0 q; q.a = a; q.P = (uint32_t)J.p[(size_t)c * J.NA + j]; q.D = (uint32_t)J.d[(size_t)c * J.NA + j];
+        const_cast<Rec0*>(s.TR)[(size_t)r * s.N + at] = q;
+        nreq[r] = at + 1u;
+        if (h->a_next == kNever) {                                  // its trace was exhausted: it has a next arrival again,
+          h->a_next = a;
+          if (h->n_active == 0u) atomicSub(J.count + 5, 1u);        // and, if it was idle, it is no longer finished
+        }
+        J.assign[(size_t)c * J.NA + j] = (int32_t)k;
+      }
+    }
+  }
+  if (k < J.K) J.tlimit[c * J.K + k] = ((uint64_t)(j + 1) < na) ? J.a[(size_t)c * J.NA + (j + 1)] : INT64_MIN;
+}
+void launch_jsq_dispatch(const SimDev& s, const JsqArgs& J, int64_t j, cudaStream_t st) {
+  k_jsq_dispatch<<<(J.C + 3) / 4, 128, 0, st>>>(s, J, (long long)j);
+}
+
 // ------------------------------------------------------------------ t_last flush (ub_per_request)
 // A request that emitted in the last executed iteration carries its t_last implicitly (== replica clock).
 __global__ void k_flush_tlast(SimDev s) {

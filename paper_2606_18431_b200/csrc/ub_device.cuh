@@ -112,6 +112,7 @@ struct StepArgs {
   uint32_t thrS, thrM;          // window size up to which a replica is queued for the S / M kernel
   const uint32_t* live;         // k_stream, list mode: the replicas to visit are live[rbeg .. rend) (else the indices themselves)
   uint32_t drift;               // this launch advances the drift group (SRPT / LAS replicas), see ub_stream.cu
+  const int64_t* tlimit;        // time fence (rule M18, JSQ): replica r runs only iterations that start before tlimit[r]; null = none
 };
 
 __device__ __forceinline__ void push_list(const StepArgs& A, uint32_t slot, uint32_t r) {

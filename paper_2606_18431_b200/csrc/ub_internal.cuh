@@ -59,7 +59,8 @@ struct __align__(16) Hdr {   // 256 bytes per replica: state (160), parameters (
   uint32_t n_completed, evict_recompute, evict_swap, swapins;
   uint32_t done, todo, n_dirty, level;  // todo: iterations of this round still to do (hand-over between kernels);
                                         // level: gamma-Ada grid level (0 for a static replica), selects the boost table
-  uint32_t pad_state[2];
+  uint32_t last_done;           // requests completed by the last executed iteration (read by the JSQ router, M18)
+  uint32_t pad_state;
   RepPar   par;               // per-replica parameters (read-only after ub_set_replicas)
   uint16_t dl[kDirtyMax];     // window positions of the re-keyed ("dirty") requests
 };
@@ -99,8 +100,14 @@ struct SimDev {                 // kernel argument (by value)
 
 // kernels (ub_step.cu, ub_aux.cu)
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, cudaStream_t st);
-void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, cudaStream_t st);
+                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, const int64_t* tlimit, cudaStream_t st);
+void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, const int64_t* tlimit,
+                cudaStream_t st);
+struct JsqArgs {                // one global arrival stream per cluster of K replicas (rule M18)
+  uint32_t K, C, NA; const int64_t* a; const int32_t* p; const int32_t* d; const uint32_t* n_arr;
+  int64_t* tlimit; int32_t* assign; uint32_t* count; int* err;
+};
+void launch_jsq_dispatch(const SimDev& s, const JsqArgs& J, int64_t j, cudaStream_t st);
 void launch_stream(const struct StepArgs& A, cudaStream_t st);    // ub_stream.cu
 void launch_debug_keys_stream(const SimDev& s, uint32_t r, uint32_t n, uint32_t* id, unsigned long long* okey, cudaStream_t st);
 void launch_gamma_ada(const SimDev& s, uint32_t rbeg, uint32_t rend, cudaStream_t st);   // ub_aux.cu

@@ -193,6 +193,8 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
   bool handed_over = false, ran = false;
 
   for (uint32_t it = 0; it < iters; it++) {
+    // time fence (JSQ router, rule M18): only iterations that start before the replica's limit run
+    if (A.tlimit && (n != 0 || next < nreq) && (n == 0 && a_next > t ? a_next : t) >= A.tlimit[r]) break;
     // ---------------- a0: idle jump + ingest (M6)
     if (n == 0) {
       if (next >= nreq) break;                  // done: this and all later iterations are no-ops
@@ -691,6 +693,7 @@ __device__ __forceinline__ void team_step(Team<WARPS>& tm, const StepArgs& A, co
           case 14: { uint32_t pk = (uint32_t)(hv >> 32); if (n > pk) pk = n; hv = (uint64_t)swap_used | ((uint64_t)pk << 32); } break;
           case 15: hv += (uint64_t)n_done + ((uint64_t)ev_nrc << 32); break;
           case 16: hv += (uint64_t)ev_nsw + ((uint64_t)swin_cnt << 32); break;
+          case 19: hv = (hv & 0xFFFFFFFF00000000ull) | (uint64_t)n_done; break;           // Hdr::last_done
           case 18: { const uint32_t q = ts->ndirty; hv = (hv & 0xFFFFFFFF00000000ull) | (q > kDirtyMax ? kDirtyMax + 1u : q); } break;
           default: break;
         }
@@ -762,7 +765,7 @@ int step_configure(uint32_t) {
 static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg,
                       uint32_t rend) {
   A.s = s; A.list = list; A.count = count; A.iters = iters; A.rbeg = rbeg; A.rend = rend; A.nstat = A.dynbase = A.tick = 0;
-  A.live = nullptr; A.drift = 0;
+  A.live = nullptr; A.drift = 0; A.tlimit = nullptr;
   const uint32_t capS = 32 * kES, capM = 128 * kEM;
   A.thrS = s.Q <= capS ? s.Q : capS - 16;
   A.thrM = s.Q <= capM ? s.Q : capM - 16;
@@ -770,19 +773,22 @@ static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* co
 }
 
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, cudaStream_t st) {
+                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, const int64_t* tlimit, cudaStream_t st) {
   StepArgs A;
   make_args(A, s, list, count, iters, rbeg, rend);
   A.tick = tick & 1u;
   A.drift = drift ? 1u : 0u;
+  A.tlimit = tlimit;
   if (live) { A.live = live; A.rbeg = 0; A.rend = nlive; }      // list mode: positions [0, nlive) of the list
   launch_stream(A, st);
 }
 
 // Runs the iterations owed by the queued replicas and empties the lists.
-void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, cudaStream_t st) {
+void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, const int64_t* tlimit,
+                cudaStream_t st) {
   StepArgs A;
   make_args(A, s, list, count, 1, rbeg, rend);
+  A.tlimit = tlimit;
   const uint32_t R = rend - rbeg;
   const uint32_t gL = R < 148u * 2 ? R : 148u * 2, gM = R < 148u * 8 ? R : 148u * 8;
   const uint32_t nS = (R + kTeamsS - 1) / kTeamsS, gS = nS < 148u * 10 ? nS : 148u * 10;

@@ -208,6 +208,10 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
       int64_t t = (int64_t)sh[0];
       int64_t a_next = (int64_t)sh[2];
       uint32_t next = (uint32_t)(sh[13] >> 32);
+      if constexpr (MULTI) {
+        // time fence (JSQ router, rule M18): only iterations that start before the replica's limit run
+        if (A.tlimit && (n != 0 || a_next != kNever) && (n == 0 && a_next > t ? a_next : t) >= __ldg(A.tlimit + r)) break;
+      }
       if (n == 0) {
         if (a_next == kNever) break;
         if (a_next > t) {
@@ -799,6 +803,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         shw[1] = H;                                                   // (kept current for a further iteration)
         shw[0] = (unsigned long long)t_end;
         if constexpr (ADA) shw[15] += (unsigned long long)n_done | ((unsigned long long)ev_nrc << 32);
+        if constexpr (MULTI) reinterpret_cast<uint32_t*>(UB_H64 + 19)[0] = n_done;   // Hdr::last_done (fenced runs: the router)
         const uint32_t pk = n > peak ? n : peak;
         shw[14] = (unsigned long long)swap_used | ((unsigned long long)pk << 32);
         if (same) atomicAdd(s.hist + (size_t)r * kTbtBins + tbt_bin(cost), same);

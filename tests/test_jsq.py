@@ -136,3 +136,35 @@ def test_bruteforce_only_the_routers_assignment_has_the_property(seed):
         if _jsq_property_holds(a[0], cand[0], t_last_of, K):
             good.append(cand[0].tolist())
     assert good == [assign[0].tolist()]
+
+
+# ------------------------------------------------------------------------------------------ GPU parity
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("policy,guard,K,C", [(W.POLICY_BOOST, 1, 4, 6), (W.POLICY_FCFS, 0, 2, 5), (W.POLICY_SRPT, 0, 3, 4),
+                                              (W.POLICY_DISTBOOST, 0, 4, 3), (W.POLICY_BOOST, 1, 32, 2)])
+def test_gpu_jsq_router_parity(policy, guard, K, C):
+    """ub_jsq_run (time-fenced runs of the step kernels + one warp per cluster for the min-reduction) against the oracle:
+    the same assignment, the same schedules."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    from paper_2606_18431_b200 import binding as B
+    n = 60 * K
+    sim = _cluster_sim(C, K, n)
+    rep = W.make_replicas(C * K, policy=policy, guard=guard, hysteresis_us=100_000 if policy == W.POLICY_BOOST else 0)
+    stream = _stream(7, C, n, gap_us=max(200, 5000 // K))
+    stream[3][-1] = n // 2                                        # (a cluster with a shorter stream)
+    o = O.OracleSim(sim, rep, _empty(sim)); oa = o.jsq_run(K, *stream)
+    g = B.Sim(sim, rep, _empty(sim)); ga = g.jsq_run(K, *stream)
+    assert np.array_equal(ga, oa)
+    assert np.array_equal(g.digest(), o.digest())
+    for x, y in zip(g.per_request(), o.per_request()):
+        assert np.array_equal(x, y)
+    gs, os_ = g.stats(), o.stats()
+    for x, y in zip(gs, os_):
+        for kk in ("iterations", "request_steps", "n_completed", "t_end_us", "done", "ttlt_us", "evict_recompute", "evict_swap"):
+            assert x[kk] == y[kk], kk
+    assert sum(s["n_completed"] for s in os_) == int(stream[3].sum())
+    assert sum(s["evict_recompute"] + s["evict_swap"] for s in os_) > 0 or K == 32
+    g.close(); o.close()
