@@ -51,7 +51,7 @@ COL = {name: i for i, name in enumerate(COLS)}
 TTLT_P99_COL = len(COLS) + 3 + 2       # ttft_us[3], then ttlt_us[2]
 
 
-def parse():
+def parse(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
@@ -65,7 +65,7 @@ def parse():
     ap.add_argument("--cpu-sample", type=int, default=64, help="replicas the one-core oracle baseline runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="headline only: no whole job, no config 2 / 3 (profiling runs)")
-    return ap.parse_args()
+    return ap.parse_args(argv)
 
 
 def peaks():
@@ -208,14 +208,26 @@ def run_reference(args):
 
 # ---------------------------------------------------------------------------------------------- the CUDA arm
 
+def torchrun_command(args, argv, port):
+    """The launch line of the contract: one rank per GPU of one node, rendezvous on 127.0.0.1."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
 def reexec_under_torchrun(args):
     """`python bench.py --gpus N` outside torchrun: launch N ranks of this script (one per GPU) and become them."""
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))
         port = s.getsockname()[1]
-    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
-           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
-    os.execv(sys.executable, cmd)
+    os.execv(sys.executable, torchrun_command(args, sys.argv[1:], port))
+
+
+def rank_layout(args, env):
+    """(rank, world, local rank) of this process; `--gpus N` must agree with the launcher's WORLD_SIZE."""
+    rank = int(env.get("RANK", "0")); world = int(env.get("WORLD_SIZE", "1")); local = int(env.get("LOCAL_RANK", "0"))
+    if args.gpus != world:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}")
+    return rank, world, local
 
 
 def stats_table(B, sim, R):
@@ -246,16 +258,40 @@ def whole_job(B, wl, traces, stream, peak, label):
             "completed": int(st[:, COL["n_completed"]].sum())}
 
 
+def gamma_ada_probe(B, w4, tr4, stream, iters=4096):
+    """Config 4 (distribution shift + memory pressure, 16384 replicas) for `iters` iterations from its loaded phase, once
+    as the static gamma sweep and once with gamma-Ada on every replica: what a round costs when UPDATEGAMMA (k_gamma_ada,
+    one CTA per replica) and the hand-over of re-keyed replicas to the team kernels (k_step) run every round."""
+    out = {}
+    R = int(w4.sim["n_replicas"])
+    for label, ada in (("static", None), ("gamma_ada", dict(window=256, min_samples=32, beta_shift=3, levels=32,
+                                                            gamma_min=0.01, gamma_max=100.0, eps_us=1000))):
+        sim = B.Sim(w4.sim, w4.replicas, tr4, stream=stream)
+        if ada:
+            sim.set_gamma_ada(ada, np.ones(R, np.uint8))
+        sim.step(150000)                                             # into the overloaded second half of the trace
+        rs0 = sum(int(st.request_steps) for st in sim.stats_raw())
+        sim.step(iters)
+        ms, rounds = sim.last_step_timing()
+        st = sim.stats_raw()
+        rs1 = sum(int(x.request_steps) for x in st)
+        out[label] = {"us_per_round": 1e3 * ms / max(1, rounds), "value": (rs1 - rs0) / (ms * 1e-3), "unit": UNIT,
+                      "mean_window": (rs1 - rs0) / max(1, iters) / R, "rounds": int(rounds)}
+        if ada:
+            out[label]["gamma_updates"] = int(sum(sim.gamma_state(r)[2] for r in range(0, R, 64)) * 64)
+        sim.close()
+    out["note"] = ("config4, 16384 replicas x 2000 requests, 4096 iterations after 150000; with adaptation on every round is "
+                   "k_gamma_ada + ub::k_stream<true,...> + the team kernels for replicas whose level changed")
+    return out
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         reexec_under_torchrun(args)
-    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.gpus != world:
-        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}")
+    rank, world, local = rank_layout(args, os.environ)
 
     # ---- synthetic traces first (the generator forks worker processes: before CUDA / NCCL are initialised).
     # Replicas are independent units, sharded over ranks by seed (weak scaling).
@@ -273,6 +309,8 @@ def main():
                           (W.config3, "config3: reasoning-heavy, 4096 replicas, MMPP-2 arrivals, swap-vs-recompute")):
             w2 = mk()
             side.append((w2, w2.traces(workers=nw), label))
+        w4 = W.config4()
+        tr4 = w4.traces(workers=nw)
 
     import torch
     import torch.distributed as dist
@@ -423,6 +461,7 @@ def main():
         if world == 1 and not args.no_extras:
             # the chat-heavy and reasoning-heavy workloads north_star names, as whole jobs
             out["workloads"] = [whole_job(B, w2, tr2, stream, peak, label) for w2, tr2, label in side]
+            out["gamma_ada"] = gamma_ada_probe(B, w4, tr4, stream)
         if not args.no_cpu_baseline and world == 1:
             n_it = args.spinup + (args.warmup + args.steps) * args.iters
             out["cpu_baseline"] = cpu_baselines(R, N, n_it, args.cpu_sample)
