@@ -517,10 +517,14 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
               // ... optionally followed, when nothing is parked, by steadily waiting requests (not resident, nothing
               // to finalise) whose first one is turned away -- on KV ("newblocked": the walk goes on over residents
               // only, of which this chunk has none left) or because the batch / token budget is used up (walk stops)
-              const bool okw = !okl && (fl & ~F_PARKED) == F_KLASS1;
               const uint32_t decm = __ballot_sync(kFull, valid && okl);
-              const uint32_t wm = pend ? 0u : __ballot_sync(kFull, valid && okw);
-              if ((decm | wm) != cv || cv == 0u || (wm != 0u && decm >= (wm & (0u - wm)))) break;   // (decoders first)
+              uint32_t wm = 0;
+              if (cv == 0u) break;
+              if (decm != cv) {                                        // (a chunk of decoders only skips all this)
+                if (pend) break;
+                wm = __ballot_sync(kFull, valid && !okl && (fl & ~F_PARKED) == F_KLASS1);
+                if ((decm | wm) != cv || decm >= (wm & (0u - wm))) break;                            // (decoders first)
+              }
               const uint32_t nv = __popc(decm);
               const uint32_t totf = __reduce_add_sync(kFull, (valid && okl) ? (r1.cached + 1u + blk_m1) >> blk_sh : 0u);
               if (crank + nv > M || carryW + nv > Tb || carryC + totf > B) break;
@@ -797,6 +801,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
 
       // ---------------- header: clock, digest (M12), cursors; counters by RED (no read needed)
       if (ndnew > kDirtyMax) ndnew = kDirtyMax + 1u;
+      __syncwarp();                                                   // every lane has read the header image (clock) by now
       if (lane == 0) {
         unsigned long long* shw = reinterpret_cast<unsigned long long*>(X.hdr[parity]);
         const uint64_t H = digest_fold(shw[1], evl, evu, t_end);
