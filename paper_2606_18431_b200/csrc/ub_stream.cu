@@ -565,6 +565,26 @@ __global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
         // ---------------- (T) behind the walk, nothing parked left: chunks of waiting requests (not resident, nothing
         // to finalise) only move up when requests in front of them completed
         if (mode != 0u && dptr >= m && !drift && c >= dlo + dspan) {
+          if (c >= 2u && c < nch && outpos == c * 32u) {
+            // the usual case, written tight: nothing in front of the tail moved, so it stays where it is and only its
+            // flags are looked at (one 4-byte read per lane and chunk); running pointers for the chunks issued ahead
+            const char* g0 = reinterpret_cast<const char*>(reinterpret_cast<const uint4*>(gE0 + (c + kRing) * 32u) + lane);
+            const ptrdiff_t dE = reinterpret_cast<const char*>(s.E1) - reinterpret_cast<const char*>(s.E0);
+            uint32_t left = n_old - c * 32u;
+            for (;;) {
+              cp_wait<kRing - 1>();
+              uint4* stg = X.ring[(c - 2u) % kRing];
+              const uint32_t fl = reinterpret_cast<const uint32_t*>(stg + 32 + lane)[3];
+              if (!__all_sync(kFull, (fl & ~F_PARKED) == F_KLASS1 || (uint32_t)lane >= left)) break;
+              if (c + kRing < nch) { cp16(stg + lane, g0); cp16(stg + 32 + lane, g0 + dE); }
+              cp_commit();
+              g0 += 512;
+              outpos += left < 32u ? left : 32u;
+              c++;
+              if (c >= nch) break;
+              left -= 32u;
+            }
+          }
           while (c < nch) {
             wait_chunk(c, outpos > c * 32u);
             const uint4* st = stage_of(c);
