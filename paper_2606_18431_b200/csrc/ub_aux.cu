@@ -275,9 +275,51 @@ __device__ int64_t radix_select(SelectSmem& sm, const int64_t* src, const Rec0* 
   return result;
 }
 
-__global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out) {
+// The same select over m values staged in shared memory (k_stats: a replica's latencies are read from HBM once and the
+// 3 x 8 passes run on chip; the first version re-read them from HBM / L2 in every pass: 466 GB of DRAM reads at
+// config 5, profiles/r02_stats.md).
+__device__ int64_t radix_select_smem(SelectSmem& sm, const unsigned long long* vals, uint32_t m, uint32_t rank0) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) { sm.prefix = 0ull; sm.rank = rank0; }
+  for (int pass = 7; pass >= 0; pass--) {
+    sm.hist[tid] = 0;
+    __syncthreads();
+    const unsigned long long prefix = sm.prefix;
+    const int sh_hi = 8 * (pass + 1);
+    for (uint32_t i = tid; i < m; i += kStatThreads) {
+      const unsigned long long v = vals[i];
+      if (pass == 7 || (v >> sh_hi) == (prefix >> sh_hi)) atomicAdd(&sm.hist[(v >> (8 * pass)) & 0xFF], 1u);
+    }
+    __syncthreads();
+    const uint32_t cntb = sm.hist[tid];
+    uint32_t inc = cntb;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { uint32_t x = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += x; }
+    if (lane == 31) sm.wtot[warp] = inc;
+    __syncthreads();
+    uint32_t off = 0;
+    for (int w = 0; w < warp; w++) off += sm.wtot[w];
+    inc += off;
+    const uint32_t exc = inc - cntb, want = sm.rank;
+    __syncthreads();
+    if (want >= exc && want < inc) {
+      sm.prefix = prefix | ((unsigned long long)tid << (8 * pass));
+      sm.rank = want - exc;
+    }
+    __syncthreads();
+  }
+  const int64_t result = (int64_t)sm.prefix;
+  __syncthreads();
+  return result;
+}
+
+constexpr uint32_t kStatSmemVals = 16384;        // latencies of one replica staged in shared memory (128 KB); longer rows use HBM
+
+__global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out, uint32_t cap) {
   __shared__ SelectSmem sm;
   __shared__ uint32_t wtot[kStatThreads / 32];
+  __shared__ uint32_t fill;
+  extern __shared__ __align__(16) unsigned long long vals[];    // [cap]
   const uint32_t r = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t tr = s.hdr[r].par.trace_id, nreq = s.n_req[tr];
@@ -290,13 +332,29 @@ __global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out)
 
   for (int which = 0; which < 2; which++) {
     const int64_t* src = which == 0 ? tf : tl;
+    const bool staged = m <= cap;
+    if (staged && m > 0) {                       // the completed requests' latencies -> shared memory, once (any order)
+      if (tid == 0) fill = 0u;
+      __syncthreads();
+      for (uint32_t base = 0; base < nreq; base += kStatThreads) {
+        const uint32_t i = base + tid;
+        const bool done = i < nreq && (ne[i] & kDoneBit);
+        const uint32_t bm = __ballot_sync(0xffffffffu, done);
+        uint32_t off = 0;
+        if (lane == 0 && bm) off = atomicAdd(&fill, (uint32_t)__popc(bm));
+        off = __shfl_sync(0xffffffffu, off, 0);
+        if (done) vals[off + __popc(bm & ((1u << lane) - 1u))] = (unsigned long long)(src[i] - TR[i].a);
+      }
+      __syncthreads();
+    }
     for (int k = 0; k < 3; k++) {
       int64_t result = 0;
       if (m > 0) {
         uint64_t rank = ((uint64_t)pct[k] * m + 99) / 100;
         if (rank < 1) rank = 1;
         if (rank > m) rank = m;
-        result = radix_select(sm, src, TR, ne, nreq, (uint32_t)(rank - 1));
+        result = staged ? radix_select_smem(sm, vals, m, (uint32_t)(rank - 1))
+                        : radix_select(sm, src, TR, ne, nreq, (uint32_t)(rank - 1));
       }
       if (tid == 0) { if (which == 0) out[r].ttft[k] = result; else out[r].ttlt[k] = result; }
     }
@@ -334,7 +392,16 @@ __global__ void __launch_bounds__(kStatThreads) k_stats(SimDev s, StatsDev* out)
   }
 }
 
-void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st) { k_stats<<<s.R, kStatThreads, 0, st>>>(s, out); }
+void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st) {
+  const uint32_t cap = s.N < kStatSmemVals ? s.N : kStatSmemVals;
+  const size_t bytes = (size_t)cap * sizeof(unsigned long long);
+  static size_t configured = 0;
+  if (bytes > configured) {
+    cudaFuncSetAttribute(k_stats, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    configured = bytes;
+  }
+  k_stats<<<s.R, kStatThreads, bytes, st>>>(s, out, cap);
+}
 
 // ------------------------------------------------------------------ richer reductions
 // Percentile curves (Fig. 6): nearest-rank percentiles at arbitrary per-mille points, rank =
