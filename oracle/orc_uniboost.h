@@ -15,7 +15,7 @@
  * and hysteresis (Eq. 7), Sec. 3.3 MemGuard (PAPER.md:198-215,
  * Eq. 8), on top of the per-iteration cost model that BASELINE.json states
  * (config 1 and config 3).  Where the paper is silent the readings are the
- * ones listed in DESIGN.md Sec. 3 (model rules M1..M14, readings G1..G24; M13 =
+ * ones listed in DESIGN.md Sec. 3 (model rules M1..M18, readings G1..G28; M13 =
  * gamma-Ada, Eq. 9 / UPDATEGAMMA; M14 = DistBoost,
  * Eq. 3-6; baselines SJF / SPF as static keys).
  * The method is a policy (a heuristic driven by a priority rule), not a
@@ -39,7 +39,14 @@
  *   tests/test_gamma_ada_pins.py: Eq. 9 on an exactly exponential tail, the
  *   log-spaced grid, no update == static gamma, the update rule re-derived every
  *   iteration; tests/test_reductions.py: numpy inverted_cdf at per-mille points
- *   and plain counts (percentile curve, SLO attainment).
+ *   and plain counts (percentile curve, SLO attainment);
+ *   hand-worked goldens G, G2, H, I, J (PHASE signal, AUTO swap rule, swap-time rounding, one-token prefill tail);
+ *   tests/test_class_reductions.py: preemption times (M15) read off the hand-derived schedules, the one-block
+ *   closed form (t_last - t_first) - (D-1) c0, class filter + numpy inverted_cdf; tests/test_oracle_pins.py
+ *   test_sarathi_*: Lindley recursion, round-robin structure, DistBoost at gamma = inf (M16);
+ *   tests/test_prefix_cache.py: the signal max(w, s_pre - h) tracked per iteration, work balance (M17);
+ *   tests/test_jsq.py: brute force over all assignments, post-hoc recount of the queue lengths, burst = round robin,
+ *   one replica per cluster = plain trace (M18).
  * Parity UNPINNED: the paper's latency tables (Tables 2-10) -- they need real
  * GPUs, model weights and datasets that are not available.
  */
