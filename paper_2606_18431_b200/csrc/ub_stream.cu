@@ -28,7 +28,7 @@
 
 namespace ub {
 
-constexpr int kSWarps = 4;                 // warps per CTA, each streams its own replicas
+constexpr int kSWarps = 2;                 // warps per CTA, each streams its own replicas
 constexpr int kRing = 4;                   // chunks in flight behind the two speculative ones
 constexpr uint32_t kFull = 0xffffffffu;
 constexpr uint32_t kEvSmem = 30;            // per-request events of one iteration kept in shared memory (spare words of skb[2..31])
@@ -109,7 +109,7 @@ __device__ __noinline__ bool drift_out_of_order(const uint64_t comp, uint64_t& k
 // over their list beside the main one: the extra re-key rule and its state stay out of the main instance, whose
 // register budget and instruction-cache footprint decide the headline number.
 template <bool ADA, bool MULTI, bool LIST, bool DRIFT>
-__global__ void __launch_bounds__(32 * kSWarps, 5) k_stream(const StepArgs A) {
+__global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
   __shared__ WarpBuf wbuf[kSWarps];
   const SimDev& s = A.s;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
