@@ -146,3 +146,16 @@ def test_gpu_starvation_shape_short_vs_long(gpu):
                 assert np.array_equal(x, y)
     assert o.class_percentiles(1, 1001, 1 << 30, pm)[1].sum() > 0
     g.close(); o.close()
+
+
+@pytest.mark.gpu
+def test_gpu_class_percentiles_argument_checks(gpu):
+    wl = pressure_workload(0, n=40)
+    g = gpu.Sim(wl.sim, wl.replicas, wl.traces())
+    for which, lo, hi, pm in ((3, 0, 10, [500]), (0, 10, 5, [500]), (1, 0, 10, [0]), (1, 0, 10, [1001]), (1, 0, 10, list(range(1, 18)))):
+        with pytest.raises(gpu.UbError) as e:
+            g.class_percentiles(which, lo, hi, pm)
+        assert e.value.code == gpu.UB_EINVAL
+    out, cnt, tot = g.class_percentiles(2, 0, 1 << 30, [500, 1000])      # nothing has run: empty classes
+    assert not out.any() and not cnt.any() and not tot.any()
+    g.close()

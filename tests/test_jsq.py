@@ -168,3 +168,35 @@ def test_gpu_jsq_router_parity(policy, guard, K, C):
     assert sum(s["n_completed"] for s in os_) == int(stream[3].sum())
     assert sum(s["evict_recompute"] + s["evict_swap"] for s in os_) > 0 or K == 32
     g.close(); o.close()
+
+
+@pytest.mark.gpu
+def test_gpu_jsq_router_rejects_wrong_states():
+    """ub_jsq_run wants clusters that tile the replicas, empty traces, no iteration run; a replica row that is too
+    short for what the router sends it is an error, not an overrun."""
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    from paper_2606_18431_b200 import binding as B
+    C, K, n = 2, 3, 40
+    stream = _stream(9, C, n)
+    sim = _cluster_sim(C, K, n)
+    g = B.Sim(sim, W.make_replicas(C * K), _empty(sim))
+    with pytest.raises(B.UbError) as e:                      # 4 does not divide the 6 replicas into 2 clusters
+        g.jsq_run(4, *stream)
+    assert e.value.code == B.UB_EINVAL
+    bad = (stream[0][:, ::-1].copy(), stream[1], stream[2], stream[3])
+    with pytest.raises(B.UbError) as e:                      # arrivals must be sorted, as for ub_load_trace
+        g.jsq_run(K, *bad)
+    assert e.value.code == B.UB_EUNSORTED
+    g.jsq_run(K, *stream)                                    # fine
+    with pytest.raises(B.UbError) as e:                      # ... but only once: the traces are no longer empty
+        g.jsq_run(K, *stream)
+    assert e.value.code == B.UB_ESTATE
+    g.close()
+    small = _cluster_sim(C, K, 4)                            # rows of 4 requests for 40 arrivals over 3 replicas
+    g = B.Sim(small, W.make_replicas(C * K), _empty(small))
+    with pytest.raises(B.UbError) as e:
+        g.jsq_run(K, *stream)
+    assert e.value.code == B.UB_EINVAL
+    g.close()
