@@ -251,7 +251,9 @@ int  ub_preempt_time(ub_sim*, int64_t* t_preempt_us, int on_device);
  * tie (one warp per cluster: a min-reduction over the cluster's replicas), and is appended to that replica's trace.
  * After the last arrival every replica runs to completion (ub_run).  assign (host, nullable): [n_clusters][max_arrivals],
  * the replica number within the cluster each arrival joined (-1 = no arrival).  Errors as ub_load_trace for the streams;
- * UB_EINVAL if a replica's row overflows; UB_ESTATE on a handle that is not in the state above.  Synchronises. */
+ * UB_EINVAL if a replica's row overflows; UB_ESTATE on a handle that is not in the state above.  Afterwards the
+ * replicas' traces hold what the router sent them: ub_set_replicas rewinds to a plain (uncoupled) run of those traces.
+ * Synchronises. */
 int  ub_jsq_run(ub_sim*, uint32_t cluster_size, uint32_t n_clusters, uint32_t max_arrivals, const int64_t* arrival_us,
                 const int32_t* prompt_tok, const int32_t* decode_tok, const uint32_t* n_arrivals, int32_t* assign);
 
