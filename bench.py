@@ -250,7 +250,14 @@ def whole_job(B, wl, traces, stream, peak, label):
     t_stats = time.perf_counter() - t1
     rs = int(st[:, COL["request_steps"]].sum()); its = int(st[:, COL["iterations"]].sum())
     sim.close()
-    return {"workload": label, "replicas": R, "value": rs / (ms * 1e-3), "unit": UNIT,
+    # the same job with 16 iterations per launch (resident-state mode: same schedules, the mode for small configurations)
+    sim = B.Sim(wl.sim, wl.replicas, traces, stream=stream, iters_per_launch=RESIDENT_IPL)
+    sim.run()
+    ms16, _ = sim.last_step_timing()
+    rs16 = int(stats_table(B, sim, R)[:, COL["request_steps"]].sum())
+    sim.close()
+    assert rs16 == rs, "the schedule must not depend on iters_per_launch"
+    return {"workload": label, "value_resident": rs16 / (ms16 * 1e-3), "resident_iters_per_launch": RESIDENT_IPL, "replicas": R, "value": rs / (ms * 1e-3), "unit": UNIT,
             "roofline_frac": rs * ALG_BYTES_PER_REQUEST_STEP / (ms * 1e-3) / 1e9 / peak,
             "request_steps": rs, "device_ms": ms, "wall_s": wall, "iterations_issued": int(issued),
             "iterations_executed_max": int(st[:, COL["iterations"]].max()), "rounds_launched": int(launches),
