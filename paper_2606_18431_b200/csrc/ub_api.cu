@@ -38,14 +38,15 @@ struct ub_sim {
   std::vector<int64_t> h_lut;            // all tables back to back
   std::vector<uint32_t> h_lut_off, h_lut_nb;
   cudaEvent_t ev0, ev1;
-  cudaStream_t aux[3]; cudaEvent_t ev_fork, ev_join[3];   // extra streams: the parts of a round overlap their tails
-  uint32_t nsplit;
+  cudaStream_t aux[ub::kMaxSplit - 1]; cudaEvent_t ev_fork, ev_join[ub::kMaxSplit - 1];   // extra streams: the parts of a round overlap their tails
+  uint32_t nsplit, ndsplit;     // parts of the main group / of the drift group (together <= kMaxSplit)
   uint32_t round_no;            // launches alternate between two ticket counters
   float last_ms; uint32_t last_launches;
 };
 
 #define CK(x) do { if ((x) != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; } } while (0)
 
+static int compact_live(ub_sim* s, uint64_t* live, bool any_state);
 static int set_dev(const ub_sim* s) { return cudaSetDevice(s->cfg.device) == cudaSuccess ? UB_OK : UB_ECUDA; }
 
 const char* ub_strerror(int e) {
@@ -92,7 +93,12 @@ int ub_create(const ub_config* c, ub_sim** out) {
   s->d_TR = nullptr; s->d_lut = nullptr;
   s->last_ms = 0.f; s->last_launches = 0;
   s->use_list = false; s->ndrift = 0; s->drift_livecnt = 0;
-  s->nsplit = c->n_replicas >= 8192 ? 2 : 1;          // (at most kMaxSplit - 1: the last set of lists is the drift group's)          // (measured on config 5: 2 parts 5.9e10, 4 parts 5.5e10 request-steps/s)
+  // parts of a round (each on a stream of its own; together with the drift group's at most kMaxSplit).  Measured: config 5
+  // (65536 replicas) 2 parts 5.9e10, 4 parts 5.5e10 request-steps/s; config 3 (4096 replicas, whole job) 1 part 1.18e10,
+  // 2 parts 1.31e10, 4 parts 1.22e10 at one iteration per launch and 2.61e10 / 3.29e10 / 3.34e10 at 64; config 2 (3072
+  // replicas) is 3 % slower in two parts than in one
+  s->nsplit = c->n_replicas >= 4096 ? 2 : 1;
+  s->ndsplit = 1;
   const size_t R = c->n_replicas, Q = c->queue_cap, N = c->max_requests, NT = c->n_traces;
   int rc = UB_OK;
   if ((rc = dmalloc(&s->d_E0, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_E1, R * Q + kWindowPad)) || (rc = dmalloc(&s->d_hdr, R)) ||
@@ -107,14 +113,17 @@ int ub_create(const ub_config* c, ub_sim** out) {
   }
   if (cudaMallocHost((void**)&s->h_word, (3 + kMaxSplit) * sizeof(unsigned long long)) != cudaSuccess ||
       cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess ||
-      cudaStreamCreateWithFlags(&s->aux[0], cudaStreamNonBlocking) != cudaSuccess ||
-      cudaStreamCreateWithFlags(&s->aux[1], cudaStreamNonBlocking) != cudaSuccess ||
-      cudaStreamCreateWithFlags(&s->aux[2], cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&s->ev_join[0], cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&s->ev_join[1], cudaEventDisableTiming) != cudaSuccess ||
-      cudaEventCreateWithFlags(&s->ev_join[2], cudaEventDisableTiming) != cudaSuccess ||
       step_configure(c->queue_cap) != 0) {
+    cudaGetLastError();
+    ub_destroy(s);
+    return UB_ECUDA;
+  }
+  bool aux_ok = true;
+  for (uint32_t i = 0; i + 1 < kMaxSplit; i++)
+    aux_ok = aux_ok && cudaStreamCreateWithFlags(&s->aux[i], cudaStreamNonBlocking) == cudaSuccess &&
+             cudaEventCreateWithFlags(&s->ev_join[i], cudaEventDisableTiming) == cudaSuccess;
+  if (!aux_ok) {
     cudaGetLastError();
     ub_destroy(s);
     return UB_ECUDA;
@@ -147,7 +156,7 @@ void ub_destroy(ub_sim* s) {
   if (s->ev0) cudaEventDestroy(s->ev0);
   if (s->ev1) cudaEventDestroy(s->ev1);
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
-  for (int i = 0; i < 3; i++) {
+  for (uint32_t i = 0; i + 1 < kMaxSplit; i++) {
     if (s->ev_join[i]) cudaEventDestroy(s->ev_join[i]);
     if (s->aux[i]) cudaStreamDestroy(s->aux[i]);
   }
@@ -331,6 +340,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   CK(cudaStreamSynchronize(s->stream));
   CK(cudaGetLastError());
   s->have_reps = true;
+  if (s->ndrift) { uint64_t all = 0; return compact_live(s, &all, true); }      // main group and drift group each from a list
   return UB_OK;
 }
 
@@ -339,54 +349,70 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
 // part finish, the other parts' CTAs already fill the freed SMs.
 // tlimit (device, [R], nullable): a fenced run (JSQ router, rule M18) -- one launch in which every replica executes the
 // iterations that start before its limit.
+// A part of a round: positions [rb, re) of the replicas themselves or of a list, its stream and its set of work lists.
+struct RoundPart { uint32_t rb, re; const uint32_t* list; bool drift; cudaStream_t st; uint32_t slot; };
+
+static uint32_t round_parts(ub_sim* s, bool ada, RoundPart* P) {
+  const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
+  const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
+  const bool lst = s->use_list && !ada;
+  uint32_t np = 0;
+  for (uint32_t i = 0; i < ns; i++) {
+    const uint32_t rb = i * part < R ? i * part : R, re = (i + 1 == ns) ? R : ((i + 1) * part < R ? (i + 1) * part : R);
+    RoundPart q;
+    q.rb = rb; q.re = re; q.list = nullptr; q.drift = false; q.slot = i; q.st = i ? s->aux[i - 1] : s->stream;
+    if (lst) { q.list = s->d_live + rb; q.rb = 0; q.re = s->livecnt[i]; }
+    if (q.re > q.rb) P[np++] = q;                  // (a part whose replicas have all finished is left out)
+  }
+  // the drift group (SRPT / LAS replicas) is one more independent set of replicas: its launches go to streams of their
+  // own beside the main parts, with the sets of work lists and counters behind theirs
+  const uint32_t nd = ada ? 0u : (lst ? s->drift_livecnt : s->ndrift);
+  if (nd) {
+    const uint32_t nds = s->ndsplit, dpart = (nd + nds - 1) / nds;
+    for (uint32_t j = 0; j < nds && j * dpart < nd; j++) {
+      RoundPart q;
+      q.rb = j * dpart; q.re = (j + 1) * dpart < nd ? (j + 1) * dpart : nd;
+      q.list = lst ? s->d_drift_live : s->d_drift; q.drift = true; q.slot = ns + j; q.st = s->aux[ns + j - 1];
+      P[np++] = q;
+    }
+  }
+  return np;
+}
+
 static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches, const int64_t* tlimit = nullptr) {
   const bool ada = s->d_ada_ring != nullptr;         // UPDATEGAMMA opens every iteration: one iteration per launch
   constexpr uint32_t kFenced = 1u << 20;             // iterations a fenced launch may run (the fence ends it long before)
   if (tlimit) n_iters = kFenced;
   const uint32_t ipl = tlimit ? kFenced : ((!ada && s->cfg.iters_per_launch > 1) ? s->cfg.iters_per_launch : 1);
-  const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
-  const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
-  // the drift group (SRPT / LAS replicas) is one more independent set of replicas: its launches go to a stream of their
-  // own beside the parts, with the last set of work lists and counters
-  constexpr uint32_t DP = kMaxSplit - 1;
-  const bool lst = s->use_list && !ada;
-  const uint32_t nd = ada ? 0u : (lst ? s->drift_livecnt : s->ndrift);
-  const uint32_t* dlist = lst ? s->d_drift_live : s->d_drift;
-  cudaStream_t dst = s->aux[2];
+  const size_t R = s->cfg.n_replicas;
+  RoundPart P[kMaxSplit];
+  const uint32_t np = round_parts(s, ada, P);
   uint32_t nl = 0;
-  if (ns > 1 || nd) {
+  bool forked = false;
+  for (uint32_t i = 0; i < np; i++) forked = forked || P[i].st != s->stream;
+  if (forked) {
     CK(cudaEventRecord(s->ev_fork, s->stream));
-    for (uint32_t i = 1; i < ns; i++) CK(cudaStreamWaitEvent(s->aux[i - 1], s->ev_fork, 0));
-    if (nd) CK(cudaStreamWaitEvent(dst, s->ev_fork, 0));
+    for (uint32_t i = 0; i < np; i++) if (P[i].st != s->stream) CK(cudaStreamWaitEvent(P[i].st, s->ev_fork, 0));
   }
   while (n_iters > 0) {
     const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
-    for (uint32_t i = 0; i < ns; i++) {
-      const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
-      if (ada) launch_gamma_ada(s->dev, rb, re, i ? s->aux[i - 1] : s->stream);
-      launch_step(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, k, rb, re, s->round_no,
-                  lst ? s->d_live + rb : nullptr, lst ? s->livecnt[i] : 0u, false, tlimit, i ? s->aux[i - 1] : s->stream);
+    n_iters -= k;
+    for (uint32_t i = 0; i < np; i++) {
+      const RoundPart& q = P[i];
+      uint32_t* list = s->d_list + 4 * R * q.slot;
+      uint32_t* count = s->d_count + 8 * q.slot;
+      if (ada) launch_gamma_ada(s->dev, q.rb, q.re, q.st);
+      launch_step(s->dev, list, count, k, q.rb, q.re, s->round_no, q.list, q.drift, tlimit, q.st);
+      // what k_stream queued for the team kernels runs at the end of the call (all owed iterations at once); with
+      // gamma-Ada after every round, because UPDATEGAMMA sits between the iterations
+      if (ada || n_iters == 0) flush_slow(s->dev, list, count, q.rb, q.re, tlimit, q.st);
     }
-    if (nd) launch_step(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, k, 0, nd, s->round_no, dlist, nd, true, tlimit, dst);
-    n_iters -= k; nl++; s->round_no++;
-    // what k_stream queued for the team kernels runs at the end of the call (all owed iterations at once); with
-    // gamma-Ada after every round, because UPDATEGAMMA sits between the iterations
-    if (ada || n_iters == 0) {
-      for (uint32_t i = 0; i < ns; i++) {
-        const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
-        flush_slow(s->dev, s->d_list + 4 * (size_t)R * i, s->d_count + 8 * i, rb, re, tlimit, i ? s->aux[i - 1] : s->stream);
-      }
-      if (nd) flush_slow(s->dev, s->d_list + 4 * (size_t)R * DP, s->d_count + 8 * DP, 0, nd, tlimit, dst);
-    }
+    nl++; s->round_no++;
   }
-  if (ns > 1 || nd) {
-    for (uint32_t i = 1; i < ns; i++) {
-      CK(cudaEventRecord(s->ev_join[i - 1], s->aux[i - 1]));
-      CK(cudaStreamWaitEvent(s->stream, s->ev_join[i - 1], 0));
-    }
-    if (nd) {
-      CK(cudaEventRecord(s->ev_join[2], dst));
-      CK(cudaStreamWaitEvent(s->stream, s->ev_join[2], 0));
+  if (forked) {
+    for (uint32_t i = 0; i < np; i++) if (P[i].st != s->stream) {
+      CK(cudaEventRecord(s->ev_join[P[i].slot - 1], P[i].st));
+      CK(cudaStreamWaitEvent(s->stream, s->ev_join[P[i].slot - 1], 0));
     }
   }
   *launches = nl;
@@ -418,15 +444,17 @@ int ub_step(ub_sim* s, uint32_t n_iters, uint64_t* live) {
 
 // The unfinished replicas of every part of a round, compacted on the device; *live = how many.  From then on the
 // streaming kernel visits only these (a finished replica never comes back, so the list stays a superset of the live
-// replicas until it is rebuilt; ub_set_replicas drops it).
-static int compact_live(ub_sim* s, uint64_t* live) {
+// replicas until it is rebuilt).  any_state: finished or not -- the lists then only separate the main group from the
+// drift group (a job that has both starts with them: a main-group warp that only skips a drift replica would still
+// hold its place on the SM beside the drift group's launch).
+static int compact_live(ub_sim* s, uint64_t* live, bool any_state) {
   const uint32_t R = s->cfg.n_replicas, ns = s->nsplit;
   const uint32_t part = ns > 1 ? (R / ns + 3) / 4 * 4 : R;
   for (uint32_t i = 0; i < ns; i++) {
     const uint32_t rb = i * part, re = (i + 1 == ns) ? R : (i + 1) * part;
-    launch_compact_live(s->dev, rb, re, nullptr, false, s->d_live + rb, s->d_livecnt + i, s->stream);
+    launch_compact_live(s->dev, rb, re, nullptr, false, any_state, s->d_live + rb, s->d_livecnt + i, s->stream);
   }
-  launch_compact_live(s->dev, 0, s->ndrift, s->d_drift, true, s->d_drift_live, s->d_livecnt + ns, s->stream);
+  launch_compact_live(s->dev, 0, s->ndrift, s->d_drift, true, any_state, s->d_drift_live, s->d_livecnt + ns, s->stream);   // (ns < kMaxSplit)
   uint32_t* hc = reinterpret_cast<uint32_t*>(s->h_word + 2);
   CK(cudaMemcpyAsync(hc, s->d_livecnt, (ns + 1) * sizeof(uint32_t), cudaMemcpyDeviceToHost, s->stream));
   CK(cudaStreamSynchronize(s->stream));
@@ -470,7 +498,7 @@ int ub_run(ub_sim* s, uint64_t max_iters, uint64_t* iters_done) {
     if (live == R) { if (chunk < 4096) chunk *= 2; }
     else {
       chunk = 512;
-      if (!ada && live > 0 && live * 8 < R * 7 && (rc = compact_live(s, &live))) return rc;
+      if (!ada && live > 0 && live * 8 < R * 7 && (rc = compact_live(s, &live, false))) return rc;
     }
   }
   s->last_ms = total_ms; s->last_launches = total_launches;
@@ -994,7 +1022,8 @@ int ub_jsq_run(ub_sim* s, uint32_t K, uint32_t C, uint32_t NA, const int64_t* a,
   J.count = s->d_count; J.err = derr;
   // arrival by arrival: [route arrival j - 1, move the fences to arrival j] -> [every replica runs the iterations that
   // start before its fence]; clusters are the batch dimension
-  s->use_list = false;
+  s->use_list = false;                             // (a replica that has drained its trace may be routed more)
+  if (s->ndrift) { uint64_t all = 0; if ((rc = compact_live(s, &all, true))) { cleanup(); return rc; } }
   for (int64_t j = 0; j <= (int64_t)maxn && rc == UB_OK; j++) {
     launch_jsq_dispatch(s->dev, J, j - 1, s->stream);
     if (j < (int64_t)maxn) { uint32_t nl = 0; rc = issue_steps(s, 0, &nl, dl); }

@@ -134,8 +134,8 @@ void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* li
 // that belong to the drift group (SRPT / LAS) or to the main one, compacted (ub_run's tail: the streaming kernel then
 // visits only these).  A replica is finished when its trace is exhausted and nothing is active (M6); finished
 // replicas never come back.
-__global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, const uint32_t* in, uint32_t drift_group, uint32_t* out,
-                               uint32_t* cnt) {
+__global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, const uint32_t* in, uint32_t drift_group, uint32_t any_state,
+                               uint32_t* out, uint32_t* cnt) {
   const uint32_t lane = threadIdx.x & 31u;
   for (uint32_t base = rbeg + (blockIdx.x * blockDim.x + threadIdx.x - lane); base < rend; base += gridDim.x * blockDim.x) {
     const uint32_t i = base + lane;
@@ -147,7 +147,7 @@ __global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, const uin
       const RepPar& q = h->par;
       const uint32_t dg = (!s.ada_ring && (q.policy == 1u || q.policy == 3u) && q.signal_mode == 0u && q.quant_mode == 0u &&
                            s.blk_shift < 32u) ? 1u : 0u;
-      alive = !(h->n_active == 0u && h->a_next == kNever) && dg == drift_group;
+      alive = (any_state || !(h->n_active == 0u && h->a_next == kNever)) && dg == drift_group;
     }
     const uint32_t m = __ballot_sync(0xffffffffu, alive);
     uint32_t off = 0;
@@ -156,10 +156,10 @@ __global__ void k_compact_live(SimDev s, uint32_t rbeg, uint32_t rend, const uin
     if (alive) out[off + __popc(m & ((1u << lane) - 1u))] = r;
   }
 }
-void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, const uint32_t* in, bool drift_group, uint32_t* out,
-                         uint32_t* cnt, cudaStream_t st) {
+void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, const uint32_t* in, bool drift_group, bool any_state,
+                         uint32_t* out, uint32_t* cnt, cudaStream_t st) {
   cudaMemsetAsync(cnt, 0, sizeof(uint32_t), st);
-  if (rend > rbeg) k_compact_live<<<148, 256, 0, st>>>(s, rbeg, rend, in, drift_group ? 1u : 0u, out, cnt);
+  if (rend > rbeg) k_compact_live<<<148, 256, 0, st>>>(s, rbeg, rend, in, drift_group ? 1u : 0u, any_state ? 1u : 0u, out, cnt);
 }
 
 // ------------------------------------------------------------------ JSQ router (rule M18; Table 9)

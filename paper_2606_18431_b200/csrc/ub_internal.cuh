@@ -66,7 +66,7 @@ struct __align__(16) Hdr {   // 256 bytes per replica: state (160), parameters (
 };
 static_assert(sizeof(Hdr) == 256 && offsetof(Hdr, par) == 160, "Hdr: 160 bytes of state, then parameters and dirty list");
 
-constexpr uint32_t kMaxSplit = 4;     // parts (streams) a scheduler round may be issued as
+constexpr uint32_t kMaxSplit = 16;    // parts (streams) a scheduler round may be issued as, the drift group's included
 constexpr uint32_t kWindowPad = 64;   // records allocated behind the last window (speculative chunk reads)
 
 struct __align__(16) AdaState { int64_t gamma_u; unsigned long long n_updates; uint32_t level, seen, on, pad; };
@@ -100,7 +100,7 @@ struct SimDev {                 // kernel argument (by value)
 
 // kernels (ub_step.cu, ub_aux.cu)
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, const int64_t* tlimit, cudaStream_t st);
+                 uint32_t tick, const uint32_t* live, bool drift, const int64_t* tlimit, cudaStream_t st);
 void flush_slow(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t rbeg, uint32_t rend, const int64_t* tlimit,
                 cudaStream_t st);
 struct JsqArgs {                // one global arrival stream per cluster of K replicas (rule M18)
@@ -117,8 +117,8 @@ void launch_pack_validate(const int64_t* a, const int32_t* p, const int32_t* d, 
                           uint32_t NT, uint32_t N, uint32_t B, uint32_t blk, Rec0* out, int* err, cudaStream_t st);
 void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t st);
 void launch_count_live(const uint32_t* count, uint32_t R, unsigned long long* live, cudaStream_t st);
-void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, const uint32_t* in, bool drift_group, uint32_t* out,
-                         uint32_t* cnt, cudaStream_t st);
+void launch_compact_live(const SimDev& s, uint32_t rbeg, uint32_t rend, const uint32_t* in, bool drift_group, bool any_state,
+                         uint32_t* out, uint32_t* cnt, cudaStream_t st);
 void launch_flush_tlast(const SimDev& s, cudaStream_t st);
 struct StatsDev {               // device-side result of the percentile reduction, one per replica
   int64_t ttft[3], ttlt[3], tbt[3];

@@ -773,13 +773,13 @@ static void make_args(StepArgs& A, const SimDev& s, uint32_t* list, uint32_t* co
 }
 
 void launch_step(const SimDev& s, uint32_t* list, uint32_t* count, uint32_t iters, uint32_t rbeg, uint32_t rend,
-                 uint32_t tick, const uint32_t* live, uint32_t nlive, bool drift, const int64_t* tlimit, cudaStream_t st) {
+                 uint32_t tick, const uint32_t* live, bool drift, const int64_t* tlimit, cudaStream_t st) {
   StepArgs A;
   make_args(A, s, list, count, iters, rbeg, rend);
   A.tick = tick & 1u;
   A.drift = drift ? 1u : 0u;
   A.tlimit = tlimit;
-  if (live) { A.live = live; A.rbeg = 0; A.rend = nlive; }      // list mode: positions [0, nlive) of the list
+  A.live = live;                                                // list mode: positions [rbeg, rend) of the list
   launch_stream(A, st);
 }
 
