@@ -350,6 +350,18 @@ def test_split_rounds_and_resident_mode(gpu, oracle_mod, ipl):
                        [0, 1, 2047, 4094, 4095, 4096, 4097, 6000, 8190, 8191], ipl=ipl)
 
 
+@pytest.mark.parametrize("ipl", [1, 16])
+def test_mixed_policies_in_parts(gpu, oracle_mod, ipl):
+    """1400 seeds x {FCFS, SRPT, BOOST} = 4200 replicas: the main group runs as two parts and the SRPT replicas as the
+    drift group, each from its own list from the first round on (then compacted to the unfinished ones in the tail of
+    the run); sampled replicas of every policy at the borders of the parts against the oracle."""
+    base = W.config2(n_seeds=1400)
+    a, P, D, n = base.traces(workers=8)
+    keep = 300                                                        # a short job: the first 300 requests of every trace
+    wl = W.custom(a[:, :keep], P[:, :keep], D[:, :keep], dict(base.sim, max_requests=keep), base.replicas)
+    _full_size_sampled(gpu, oracle_mod, wl, [0, 1, 2, 2098, 2099, 2100, 2101, 2102, 3000, 3001, 4197, 4198, 4199], ipl=ipl)
+
+
 # ------------------------------------------------------------------------------------------ streaming kernel, randomised
 
 @pytest.mark.parametrize("seed", range(8))
