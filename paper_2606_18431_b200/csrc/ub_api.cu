@@ -397,7 +397,7 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches, const in
   while (n_iters > 0) {
     const uint32_t k = n_iters < ipl ? (uint32_t)n_iters : ipl;
     n_iters -= k;
-    for (uint32_t i = 0; i < np; i++) {
+    for (uint32_t i = np; i-- > 0;) {                // (the drift group first: its replica-steps are the longer ones)
       const RoundPart& q = P[i];
       uint32_t* list = s->d_list + 4 * R * q.slot;
       uint32_t* count = s->d_count + 8 * q.slot;

@@ -180,6 +180,8 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
     Rec1* gE1 = s.E1 + (size_t)r * Q;
     const bool isboost = par.policy == 2;
     const bool guard = par.guard != 0;
+    // flags of a resident in steady decode: admitted and emitting last iteration; class 0 when MemGuard locks it
+    const uint32_t okflags = F_RESIDENT | F_ADMITNOW | F_EMITPREV | (guard ? 0u : F_KLASS1);
 
     // the streaming path covers the paper's signal and quantiser under every policy but DistBoost (whose decode-queue
     // key is the request's first-token time, a gather from the per-request outputs)
@@ -496,12 +498,13 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
       };
       uint32_t c = 0;
       for (;;) {
-        // ---------------- (A) chunks of MemGuard-locked residents in steady decode (each wants one token, emits it,
-        // neither completes nor crosses its Eq. 8 threshold) that fit as a whole: class 0 in stored order (so in front
-        // of a parked request of class 1), nothing is re-keyed, every record advances by one token (M2, M7, M10)
-        if (mode == 0u && guard && !drift && c < nch) {
+        // ---------------- (A) chunks of residents in steady decode (each wants one token, emits it, neither completes
+        // nor crosses its Eq. 8 threshold) that fit as a whole: nothing is re-keyed, every record advances by one token
+        // (M2, M7, M10).  With MemGuard they are class 0 in stored order, so in front of a parked request of class 1;
+        // without it only when nothing is parked
+        if (mode == 0u && c < nch) {
           const bool pend = dptr < m;
-          if (!pend || (X.skb[dptr].y >> 31)) {
+          if (!pend || (guard && (X.skb[dptr].y >> 31))) {
             do {
               wait_chunk(c, outpos > c * 32u);
               const uint4* st = stage_of(c);
@@ -512,7 +515,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
               const bool valid = (cv >> lane) & 1u;
               const uint32_t fl = r1.flags;
               const uint32_t sig1 = r0.P + r1.d + 1u;                  // signal after this token
-              const bool okl = (fl & (F_LOCK_MASK_LOW)) == (F_RESIDENT | F_ADMITNOW | F_EMITPREV) && r1.cached + 2u == sig1 &&
+              const bool okl = (fl & (F_LOCK_MASK_LOW)) == okflags && r1.cached + 2u == sig1 &&
                                r1.d + 1u != r0.D && sig1 != (k << (fl >> F_LOCK_SHIFT));
               // ... optionally followed, when nothing is parked, by steadily waiting requests (not resident, nothing
               // to finalise) whose first one is turned away -- on KV ("newblocked": the walk goes on over residents
@@ -520,6 +523,17 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
               const uint32_t decm = __ballot_sync(kFull, valid && okl);
               uint32_t wm = 0;
               if (cv == 0u) break;
+              uint64_t klast = 0;
+              if constexpr (DRIFT) {
+                // drifting keys: the decoders' keys move together, so they keep their order among themselves; a waiting
+                // request behind them does not move with them (general path), and the first decoder must not come to
+                // sort in front of anything written so far
+                if (decm != cv) break;
+                const uint64_t comp = (guard ? 0ull : (1ull << 63)) |
+                                      ((uint64_t)(par.policy == 1 ? r0.D - r1.d - 1u : sig1) << 32) | (uint64_t)r1.id;
+                if (__shfl_sync(kFull, comp, __ffs(cv) - 1) < kmax) break;
+                klast = __shfl_sync(kFull, comp, 31 - __clz((int)cv));
+              }
               if (decm != cv) {                                        // (a chunk of decoders only skips all this)
                 if (pend) break;
                 wm = __ballot_sync(kFull, valid && !okl && (fl & ~F_PARKED) == F_KLASS1);
@@ -554,6 +568,7 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
               } else if (valid && moved) {
                 __stcg(reinterpret_cast<int4*>(gE1 + np), *reinterpret_cast<const int4*>(&c1));
               }
+              if constexpr (DRIFT) kmax = klast;
               carryW += nv; carryC += totf; carryN = crank + nv;       // (carryN: the turned-away request's rank)
               crank += __popc(cv); outpos += __popc(cv);
               mode = nmode;
@@ -564,7 +579,23 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
         }
         // ---------------- (T) behind the walk, nothing parked left: chunks of waiting requests (not resident, nothing
         // to finalise) only move up when requests in front of them completed
-        if (mode != 0u && dptr >= m && !drift && c >= dlo + dspan) {
+        bool tail = mode != 0u && dptr >= m && c >= dlo + dspan;
+        const uint32_t c_tail = c;
+        if constexpr (DRIFT) {
+          // drifting keys: a waiting request keeps its key, but one written in front of the tail may have moved behind
+          // the tail's first request (LAS).  The tail is sorted, so it may stay as it is when its first request does not
+          // sort in front of anything written so far (kmax); else the general path lists the out-of-order ones
+          if (tail && c < nch) {
+            wait_chunk(c, outpos > c * 32u);
+            const uint4* st = stage_of(c);
+            const uint4 f0 = st[0], f1 = st[32];
+            const Rec0 r0 = *reinterpret_cast<const Rec0*>(&f0);
+            const Rec1 r1 = *reinterpret_cast<const Rec1*>(&f1);
+            const uint32_t key2 = par.policy == 1 ? r0.D - r1.d : r0.P + r1.d;
+            tail = ((1ull << 63) | ((uint64_t)key2 << 32) | (uint64_t)r1.id) >= kmax;
+          }
+        }
+        if (tail) {
           if (c >= 2u && c < nch && outpos == c * 32u) {
             // the usual case, written tight: nothing in front of the tail moved, so it stays where it is and only its
             // flags are looked at (one 4-byte read per lane and chunk); running pointers for the chunks issued ahead
@@ -601,6 +632,18 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
             outpos += left < 32u ? left : 32u;
             if (c >= 2u) issue_chunk(c + kRing);
             c++;
+          }
+          if constexpr (DRIFT) {
+            if (c > c_tail && c < nch) {                              // more follows: the tail's last request is the largest so far
+              __syncwarp();
+              const int4 v0 = __ldcg(reinterpret_cast<const int4*>(gE0 + outpos - 1u));
+              const int4 v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + outpos - 1u));
+              const Rec0 r0 = *reinterpret_cast<const Rec0*>(&v0);
+              const Rec1 r1 = *reinterpret_cast<const Rec1*>(&v1);
+              const uint32_t key2 = par.policy == 1 ? r0.D - r1.d : r0.P + r1.d;
+              const uint64_t comp = (1ull << 63) | ((uint64_t)key2 << 32) | (uint64_t)r1.id;
+              if (comp > kmax) kmax = comp;
+            }
           }
         }
         if (c > nch || (c == nch && dptr >= m)) break;                // (chunk nch is empty: the parked tail)
