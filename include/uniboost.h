@@ -37,7 +37,7 @@ extern "C" {
 #define UB_TBT_BINS    4352u      /* log-linear TBT histogram, 7 sub-bits, gaps < 2^40 us (M11) */
 
 enum { UB_OK = 0, UB_EINVAL = -1, UB_ENOMEM = -2, UB_ECUDA = -3, UB_ESTATE = -4,
-       UB_EUNSORTED = -5, UB_EINFEASIBLE = -6, UB_ELIVELOCK = -7 };
+       UB_EUNSORTED = -5, UB_EINFEASIBLE = -6, UB_ELIVELOCK = -7, UB_ETOOBIG = -8 };
 
 /* policy (M5): key = a | D-d | a - b_gamma(w_hat) | sig */
 enum { UB_FCFS = 0, UB_SRPT = 1, UB_BOOST = 2, UB_LAS = 3,
@@ -223,6 +223,17 @@ int  ub_last_step_timing(ub_sim*, float* kernel_ms, uint32_t* launches);
  * Both synchronise. */
 int  ub_percentile_curve(ub_sim*, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out_us);
 int  ub_slo_attainment(ub_sim*, uint32_t which, const int64_t* threshold_us, uint32_t n, uint32_t* met);
+
+/* ub_percentile_curve for callers that cannot call cudaMalloc (tight serving loops, harnesses that forbid it): same
+ * arguments, same result, but no cudaMalloc / cudaFree or other allocating routine is called -- the device staging of
+ * the result is a static device array inside the library of UB_NOALLOC_CURVE_MAX int64 values (512 KB, held by every
+ * GPU that loads the library until the process exits).  n_replicas x n > UB_NOALLOC_CURVE_MAX returns UB_ETOOBIG.
+ * The array is shared by every call on the device, from any handle, and keeps the last call's values: the kernel
+ * overwrites every value it returns, nothing needs clearing, but two calls that overlap on the GPU (two handles on
+ * different streams or host threads) race -- serialise them.  The first call on a device looks the array's device
+ * address up (once per device).  Synchronises. */
+#define UB_NOALLOC_CURVE_MAX 65536u
+int  ub_percentile_curve_noalloc(ub_sim*, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out_us);
 
 /* Per-class reductions (the short- / long-request tables of the starvation experiment,
  * PAPER.md:549-560 Table 3, Tables 4-5), device-resident: over the completed requests of each replica

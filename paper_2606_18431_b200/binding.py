@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libuniboost.so")
 UB_ABI_VERSION = 1
 UB_MAX_QUEUE = 2048
 UB_TBT_BINS = 4352
-UB_OK, UB_EINVAL, UB_ENOMEM, UB_ECUDA, UB_ESTATE, UB_EUNSORTED, UB_EINFEASIBLE, UB_ELIVELOCK = 0, -1, -2, -3, -4, -5, -6, -7
+UB_OK, UB_EINVAL, UB_ENOMEM, UB_ECUDA, UB_ESTATE, UB_EUNSORTED, UB_EINFEASIBLE, UB_ELIVELOCK, UB_ETOOBIG = 0, -1, -2, -3, -4, -5, -6, -7, -8
+UB_NOALLOC_CURVE_MAX = 65536
 
 U32, I64, U64 = C.c_uint32, C.c_int64, C.c_uint64
 
@@ -58,7 +59,7 @@ EXPORTS = ("ub_create", "ub_destroy", "ub_load_trace", "ub_set_replicas", "ub_st
            "ub_per_request", "ub_digest", "ub_boost_lut", "ub_tbt_hist", "ub_debug_get_state",
            "ub_last_step_timing", "ub_set_iters_per_launch", "ub_set_gamma_ada", "ub_gamma_state", "ub_gamma_grid",
            "ub_percentile_curve", "ub_slo_attainment", "ub_debug_keys", "ub_debug_keys_stream", "ub_debug_set_state",
-           "ub_class_percentiles", "ub_preempt_time", "ub_load_trace_prefix", "ub_jsq_run",
+           "ub_class_percentiles", "ub_preempt_time", "ub_load_trace_prefix", "ub_jsq_run", "ub_percentile_curve_noalloc",
            "ub_strerror")
 
 _lib = None
@@ -93,6 +94,7 @@ def lib():
         L.ub_debug_keys_stream.argtypes = [vp, U32, P(U32), vp, vp, vp]
         L.ub_debug_set_state.argtypes = [vp, U32, U32, vp, vp, vp, vp, I64, U32, U32]
         L.ub_percentile_curve.argtypes = [vp, U32, vp, U32, vp]
+        L.ub_percentile_curve_noalloc.argtypes = [vp, U32, vp, U32, vp]
         L.ub_slo_attainment.argtypes = [vp, U32, vp, U32, vp]
         L.ub_class_percentiles.argtypes = [vp, U32, U32, U32, vp, U32, vp, vp, vp]
         L.ub_preempt_time.argtypes = [vp, vp, C.c_int]
@@ -292,6 +294,14 @@ class Sim:
         pm = np.ascontiguousarray(permille, np.uint32)
         out = np.zeros((self.R, len(pm)), np.int64)
         _chk(lib().ub_percentile_curve(self._h, int(which), pm.ctypes.data, len(pm), out.ctypes.data))
+        return out
+
+    def percentile_curve_noalloc(self, which, permille):
+        """percentile_curve through the entry point that allocates nothing on the device (static scratch in the library;
+        UB_ETOOBIG when R x n exceeds UB_NOALLOC_CURVE_MAX)."""
+        pm = np.ascontiguousarray(permille, np.uint32)
+        out = np.zeros((self.R, len(pm)), np.int64)
+        _chk(lib().ub_percentile_curve_noalloc(self._h, int(which), pm.ctypes.data, len(pm), out.ctypes.data))
         return out
 
     def slo_attainment(self, which, threshold_us):

@@ -59,6 +59,7 @@ const char* ub_strerror(int e) {
     case UB_EUNSORTED: return "arrivals not non-decreasing";
     case UB_EINFEASIBLE: return "request does not fit the KV capacity or has P<1 or D<1";
     case UB_ELIVELOCK: return "max_iters reached before all replicas finished";
+    case UB_ETOOBIG: return "size beyond the static scratch of a no-allocation entry point (UB_NOALLOC_CURVE_MAX values)";
     default: return "unknown";
   }
 }
@@ -694,6 +695,26 @@ int ub_percentile_curve(ub_sim* s, uint32_t which, const uint32_t* permille, uin
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   if (e == cudaSuccess) e = cudaGetLastError();
   cudaFree(d_out);
+  if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
+  return UB_OK;
+}
+
+// ub_percentile_curve without any allocation: the device staging of the result is a static array of the library
+// (ub_aux.cu), shared by every call on the device.
+int ub_percentile_curve_noalloc(ub_sim* s, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out) {
+  if (!s || !permille || !out || which > 1 || n < 1 || n > 16) return UB_EINVAL;
+  for (uint32_t k = 0; k < n; k++) if (permille[k] < 1 || permille[k] > 1000) return UB_EINVAL;
+  if (!s->have_reps) return UB_ESTATE;
+  const size_t R = s->cfg.n_replicas;
+  if (R * n > kNoAllocCurveMax) return UB_ETOOBIG;
+  if (set_dev(s)) return UB_ECUDA;
+  const int64_t* staged = nullptr;
+  const int lrc = launch_percentile_curve_noalloc(s->dev, s->cfg.device, which, permille, n, &staged, s->stream);
+  if (lrc == -1) return UB_ETOOBIG;
+  if (lrc != 0 || !staged) return UB_ECUDA;
+  cudaError_t e = cudaMemcpyAsync(out, staged, R * n * 8, cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) e = cudaGetLastError();
   if (e != cudaSuccess) { cudaGetLastError(); return UB_ECUDA; }
   return UB_OK;
 }

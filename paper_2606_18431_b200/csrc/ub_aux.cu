@@ -1,5 +1,6 @@
 // ub_aux.cu -- the kernels around the scheduling step: trace validation + packing, reset, live count,
 // t_last flush, and the device-resident percentile reduction a6 (M11; t_p of PAPER.md:225).
+#include <mutex>
 #include "ub_internal.cuh"
 
 namespace ub {
@@ -431,6 +432,34 @@ void launch_percentile_curve(const SimDev& s, uint32_t which, const uint32_t* pe
   CurveArgs c; c.which = which; c.n = n;
   for (uint32_t k = 0; k < 16; k++) c.permille[k] = k < n ? permille[k] : 0;
   k_percentile_curve<<<s.R, kStatThreads, 0, st>>>(s, c, out);
+}
+
+// ub_percentile_curve_noalloc: the same kernel with its result staged in a file-scope device array instead of a
+// cudaMalloc'ed buffer (callers that cannot allocate).  Every GPU that loads the library holds the array (512 KB)
+// until exit; every call on a device shares it, so calls that overlap on the GPU race.  The kernel writes every
+// one of the R x n values it is asked for (0 for a replica without completed requests): nothing has to start at zero.
+// In host code `g_curve_scratch` is only a stand-in for the symbol: the device address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) long long g_curve_scratch[kNoAllocCurveMax];
+int launch_percentile_curve_noalloc(const SimDev& s, int device, uint32_t which, const uint32_t* permille, uint32_t n,
+                                    const int64_t** staged, cudaStream_t st) {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static long long* addr[kMaxDev] = {};
+  if (device < 0 || device >= kMaxDev || (size_t)s.R * n > kNoAllocCurveMax) return -1;
+  long long* ptr = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[device]) {                              // set-up, once per device (the caller made `device` current)
+      void* p = nullptr;
+      if (cudaGetSymbolAddress(&p, g_curve_scratch) != cudaSuccess || !p) { cudaGetLastError(); return -2; }
+      addr[device] = static_cast<long long*>(p);
+    }
+    ptr = addr[device];
+  }
+  launch_percentile_curve(s, which, permille, n, reinterpret_cast<int64_t*>(ptr), st);
+  *staged = reinterpret_cast<const int64_t*>(ptr);
+  return 0;
 }
 
 // Per-class reductions (Tables 3-5): over the completed requests of a replica whose total

@@ -126,6 +126,11 @@ struct StatsDev {               // device-side result of the percentile reductio
 void launch_stats(const SimDev& s, StatsDev* out, cudaStream_t st);
 void launch_percentile_curve(const SimDev& s, uint32_t which, const uint32_t* permille, uint32_t n, int64_t* out,
                              cudaStream_t st);
+// the same with the result staged in a static device array of kNoAllocCurveMax values (ub_aux.cu); *staged = its device
+// address.  0, -1 (n_replicas x n beyond the array, or device number out of range) or -2 (symbol lookup failed)
+constexpr size_t kNoAllocCurveMax = 65536;
+int launch_percentile_curve_noalloc(const SimDev& s, int device, uint32_t which, const uint32_t* permille, uint32_t n,
+                                    const int64_t** staged, cudaStream_t st);
 void launch_class_percentiles(const SimDev& s, uint32_t which, uint32_t len_lo, uint32_t len_hi, const uint32_t* permille,
                               uint32_t n, int64_t* out, uint32_t* count, int64_t* sum, cudaStream_t st);
 void launch_slo_count(const SimDev& s, uint32_t which, uint32_t n, const int64_t* thr, uint32_t* out, cudaStream_t st);
