@@ -311,6 +311,10 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
     for (size_t r = 0; r < R && all; r++)
       all = reps[r].policy < UB_DISTBOOST && reps[r].signal_mode == 0 && reps[r].quant_mode == 0;
     s->dev.all_stream = all ? 1u : 0u;
+    bool bg = s->dev.blk_shift < 32u;
+    for (size_t r = 0; r < R && bg; r++)
+      bg = reps[r].policy == UB_BOOST && reps[r].guard != 0 && reps[r].signal_mode == 0 && reps[r].quant_mode == 0;
+    s->dev.all_boost_guard = bg ? 1u : 0u;
   }
   {
     // the drift group: replicas whose keys move with every token (SRPT, LAS) and that the streaming kernel covers

@@ -96,6 +96,8 @@ struct SimDev {                 // kernel argument (by value)
   uint32_t  ada_W, ada_G, ada_min, ada_shift;
   int64_t   ada_eps;
   uint32_t  all_stream;         // every replica is eligible for the streaming kernel: its rare hand-overs all go to the L team kernel
+  uint32_t  all_boost_guard;    // every replica is BOOST with MemGuard, the paper's signal and quantiser (the method itself,
+                                // PAPER.md:406-473), block size a power of two: k_stream's instance specialised for it runs
 };
 
 // kernels (ub_step.cu, ub_aux.cu)
