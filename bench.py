@@ -446,7 +446,7 @@ def main():
                        "job_replicas_gathered": int(job_stats.shape[0])},
             "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                          "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
-                         "kernel": "ub::k_stream<false,false>",
+                         "kernel": "ub::k_stream<false,false,false,false,true> (one iteration per launch, all replicas, the instance for all-BOOST-with-MemGuard jobs)",
                          "alg_bytes_per_request_step": ALG_BYTES_PER_REQUEST_STEP,
                          "request_steps_per_launch": (rs2 - rs1) / max(1, rounds),
                          "avg_launch_ms": ms / max(1, rounds),

@@ -270,8 +270,14 @@ __global__ void __launch_bounds__(32 * kSWarps, 10) k_stream(const StepArgs A) {
         if ((uint32_t)lane < nd) {
           spos = (!MULTI || it == 0) ? (uint32_t)reinterpret_cast<const Hdr*>(X.hdr[parity])->dl[lane]
                                      : (uint32_t)__ldcg(s.hdr[r].dl + lane);
-          v0 = __ldcg(reinterpret_cast<const int4*>(gE0 + spos));
-          v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + spos));
+          if ((!MULTI || it == 0) && spos < 64u) {                   // in the two chunks that came with the header: no
+            const uint4* sp = X.spec[parity][spos >> 5] + (spos & 31u);   // second trip to memory
+            const uint4 a0 = sp[0], a1 = sp[32];
+            v0 = *reinterpret_cast<const int4*>(&a0); v1 = *reinterpret_cast<const int4*>(&a1);
+          } else {
+            v0 = __ldcg(reinterpret_cast<const int4*>(gE0 + spos));
+            v1 = __ldcg(reinterpret_cast<const int4*>(gE1 + spos));
+          }
         } else if ((uint32_t)lane < m) {
           const uint32_t i = next + ((uint32_t)lane - nd);
           v0 = __ldg(reinterpret_cast<const int4*>(UB_TR + i));
