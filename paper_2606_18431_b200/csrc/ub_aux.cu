@@ -63,42 +63,59 @@ void launch_reset(const SimDev& s, uint32_t* list, uint32_t* count, cudaStream_t
 
 // ------------------------------------------------------------------ gamma-Ada (M13; Eq. 9, UPDATEGAMMA PAPER.md:588-601)
 // Launched in front of every scheduler round while adaptation is on ("gamma <- UPDATEGAMMA(S)" opens the loop of
-// Algorithm 1).  One CTA per replica; it leaves at once unless the replica adapts, is not finished, and
+// Algorithm 1).  One warp per replica; it leaves at once unless the replica adapts, is not finished, and
 // a request completed since the last update.  Then: window of the last min(W, n_completed) end-to-end latencies ->
-// shared memory, bitonic sort, nearest-rank t95 / t99, the fixed-point update, the grid level.  A level change
+// shared memory, nearest-rank t95 / t99 by selection, the fixed-point update, the grid level.  A level change
 // switches the boost table (Hdr::level) and re-keys every request: n_dirty is set to overflow, so this round's
 // ordering is rebuilt from scratch by the team kernel.
-constexpr int kAdaThreads = 128;
+constexpr int kAdaThreads = 128;                   // 4 warps, one replica each
 constexpr long long kLn5e12 = 1609437912434LL;     // floor(ln 5 * 1e12)
 
-__global__ void __launch_bounds__(kAdaThreads) k_gamma_ada(SimDev s, uint32_t rbeg) {
-  __shared__ long long v[1024];
-  const uint32_t r = rbeg + blockIdx.x;
+// One WARP per replica.  Only two order statistics near the top are wanted (nearest-rank t95 and t99 of the last
+// m <= W <= 1024 latencies), so the window is not sorted: the largest value is taken out m - r95 + 1 times (each lane
+// keeps the largest of its own strided share; a round is one 64-bit warp maximum and a re-scan by the winning lane).
+__global__ void __launch_bounds__(kAdaThreads) k_gamma_ada(SimDev s, uint32_t rbeg, uint32_t rend) {
+  __shared__ long long vs[kAdaThreads / 32][1024];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  const uint32_t r = rbeg + blockIdx.x * (kAdaThreads / 32) + warp;
+  if (r >= rend) return;
   AdaState* st = s.ada_state + r;
   if (!st->on) return;
   Hdr* h = s.hdr + r;
   const uint32_t nc = h->n_completed;
   if ((h->n_active == 0 && h->a_next == kNever) || nc == st->seen || nc < s.ada_min) return;
   const uint32_t m = nc < s.ada_W ? nc : s.ada_W;
-  uint32_t npad = 1; while (npad < m) npad <<= 1;
+  long long* v = vs[warp];
   const int64_t* ring = s.ada_ring + (size_t)r * s.ada_W;
-  for (uint32_t i = threadIdx.x; i < npad; i += kAdaThreads) v[i] = i < m ? (long long)ring[i] : INT64_MAX;
-  __syncthreads();
-  for (uint32_t kk = 2; kk <= npad; kk <<= 1)
-    for (uint32_t j = kk >> 1; j > 0; j >>= 1) {
-      for (uint32_t i = threadIdx.x; i < npad; i += kAdaThreads) {
-        const uint32_t l = i ^ j;
-        if (l > i) {
-          const long long a = v[i], b = v[l];
-          if ((a > b) == ((i & kk) == 0)) { v[i] = b; v[l] = a; }
-        }
-      }
-      __syncthreads();
+  // (latencies are >= 0: INT64_MIN marks a value that was taken out)
+  long long best = INT64_MIN; uint32_t besti = 0;
+  for (uint32_t i = lane; i < m; i += 32u) {
+    const long long x = (long long)ring[i];
+    v[i] = x;
+    if (x > best) { best = x; besti = i; }
+  }
+  uint32_t r95 = (95u * m + 99u) / 100u, r99 = (99u * m + 99u) / 100u;        // nearest rank (t_p of PAPER.md:225)
+  if (r95 < 1) r95 = 1; if (r99 < 1) r99 = 1;
+  const uint32_t k99 = m - r99 + 1u, k95 = m - r95 + 1u;                      // the k-th largest has rank m - k + 1
+  long long t99 = 0, t95 = 0;
+  for (uint32_t kk = 1; kk <= k95; kk++) {
+    // 64-bit maximum over the lanes: high words (signed), then low words (unsigned) among the lanes that hold it
+    const int hi = (int)(best >> 32);
+    const int mhi = __reduce_max_sync(0xffffffffu, hi);
+    const uint32_t lo = hi == mhi ? (uint32_t)best : 0u;
+    const uint32_t mlo = __reduce_max_sync(0xffffffffu, lo);
+    const uint32_t who = __ballot_sync(0xffffffffu, hi == mhi && (uint32_t)best == mlo);
+    const long long top = ((long long)mhi << 32) | (long long)mlo;
+    if (kk == k99) t99 = top;
+    if (kk == k95) t95 = top;
+    if (lane == (uint32_t)__ffs(who) - 1u && kk < k95) {                      // take one instance out, find my next largest
+      v[besti] = INT64_MIN;
+      best = INT64_MIN; besti = 0;
+      for (uint32_t i = lane; i < m; i += 32u) { const long long x = v[i]; if (x > best) { best = x; besti = i; } }
     }
-  if (threadIdx.x == 0) {
-    uint32_t r95 = (95u * m + 99u) / 100u, r99 = (99u * m + 99u) / 100u;      // nearest rank (t_p of PAPER.md:225)
-    if (r95 < 1) r95 = 1; if (r99 < 1) r99 = 1;
-    long long delta = v[r99 - 1] - v[r95 - 1];
+  }
+  if (lane == 0) {
+    long long delta = t99 - t95;
     if (delta < s.ada_eps) delta = s.ada_eps;
     const long long hat = kLn5e12 / delta;                                     // Eq. 9 in micro units
     long long g = st->gamma_u;
@@ -112,7 +129,8 @@ __global__ void __launch_bounds__(kAdaThreads) k_gamma_ada(SimDev s, uint32_t rb
   }
 }
 void launch_gamma_ada(const SimDev& s, uint32_t rbeg, uint32_t rend, cudaStream_t st) {
-  if (rend > rbeg) k_gamma_ada<<<rend - rbeg, kAdaThreads, 0, st>>>(s, rbeg);
+  constexpr uint32_t per = kAdaThreads / 32;
+  if (rend > rbeg) k_gamma_ada<<<(rend - rbeg + per - 1) / per, kAdaThreads, 0, st>>>(s, rbeg, rend);
 }
 
 __global__ void k_ada_init(SimDev s) {
