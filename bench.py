@@ -66,6 +66,8 @@ def parse(argv=None):
     ap.add_argument("--cpu-sample", type=int, default=64, help="replicas the one-core oracle baseline runs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="headline only: no whole job, no config 2 / 3 (profiling runs)")
+    ap.add_argument("--probe", default=None, choices=["gamma_ada"],
+                    help="run only this extra key of the bench line and print it (profiling runs: profiles/r02_gamma_ada.md)")
     return ap.parse_args(argv)
 
 
@@ -297,6 +299,15 @@ def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.probe == "gamma_ada":
+        w4 = W.config4()
+        tr4 = w4.traces(workers=max(1, min(32, os.cpu_count() or 1)))
+        import torch
+        from paper_2606_18431_b200 import binding as B
+        if not torch.cuda.is_available():
+            raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
+        print(json.dumps({"gamma_ada": gamma_ada_probe(B, w4, tr4, torch.cuda.current_stream().cuda_stream)}))
+        return
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         reexec_under_torchrun(args)
     rank, world, local = rank_layout(args, os.environ)
