@@ -362,6 +362,33 @@ def test_mixed_policies_in_parts(gpu, oracle_mod, ipl):
     _full_size_sampled(gpu, oracle_mod, wl, [0, 1, 2, 2098, 2099, 2100, 2101, 2102, 3000, 3001, 4197, 4198, 4199], ipl=ipl)
 
 
+@pytest.mark.parametrize("ipl", [1, 16])
+def test_specialised_and_generic_instances_agree(gpu, oracle_mod, ipl):
+    """A job whose replicas are all BOOST with MemGuard runs k_stream's specialised instance (bench.py's kernel); one
+    FCFS replica added to the same job forces the generic instances.  Both must give the BOOST replicas the same
+    schedule, per-request times and histograms -- and the oracle's, on sampled replicas (6000 replicas: two parts)."""
+    base = W.config5(n_seeds=6000, n_requests=400)
+    a, P, D, n = base.traces(workers=8)
+    R = base.R
+    spec = gpu.Sim(base.sim, base.replicas, (a, P, D, n), iters_per_launch=ipl)
+    rep2 = {k: np.concatenate([v, v[:1]]) for k, v in base.replicas.items()}
+    rep2["policy"][-1] = W.POLICY_FCFS; rep2["guard"][-1] = 0
+    sim2 = dict(base.sim, n_replicas=R + 1)
+    gen = gpu.Sim(sim2, rep2, (a, P, D, n), iters_per_launch=ipl)
+    spec.run(); gen.run()
+    assert np.array_equal(spec.digest(), gen.digest()[:R])
+    s1, s2 = spec.per_request(), gen.per_request()
+    for x, y in zip(s1, s2):
+        assert np.array_equal(x, y[:R])
+    assert np.array_equal(spec.tbt_hist(5), gen.tbt_hist(5)) and np.array_equal(spec.tbt_hist(R - 1), gen.tbt_hist(R - 1))
+    picks = [0, 1, 2999, 3000, 3001, 5999]
+    sub = base.select(picks)
+    o = oracle_mod.OracleSim(sub.sim, sub.replicas, tuple(x[np.unique(base.replicas["trace_id"][picks])] for x in (a, P, D, n)))
+    o.run()
+    assert np.array_equal(spec.digest()[picks], o.digest())
+    spec.close(); gen.close(); o.close()
+
+
 # ------------------------------------------------------------------------------------------ streaming kernel, randomised
 
 @pytest.mark.parametrize("seed", range(8))
