@@ -145,7 +145,11 @@ int  ub_step(ub_sim*, uint32_t n_iters, uint64_t* live_replicas);
 
 /* Algorithm 1's outer loop ("while system is running") over the whole trace: ub_step until every replica
  * has served its last request (trace exhausted and no request active, M6) or max_iters iterations were issued (then
- * UB_ELIVELOCK).  iters_done (host, nullable) = iterations issued.  Synchronises. */
+ * UB_ELIVELOCK).  iters_done (host, nullable) = iterations issued.  Synchronises.
+ * The rounds are replayed from a captured CUDA graph (64 rounds at a time) while the set of unfinished replicas a round
+ * visits is unchanged; if the handle's stream is a default stream (which cannot be captured) the graph runs on a stream
+ * of the library's, ordered behind the handle's stream and in front of it again by events.  Same schedules either way;
+ * gamma-Ada runs and a stream that refuses capture fall back to plain launches. */
 int  ub_run(ub_sim*, uint64_t max_iters, uint64_t* iters_done);
 
 /* Device-resident reduction of the per-request histories to the tail metrics the paper reports (TTFT, TTLT = E2E

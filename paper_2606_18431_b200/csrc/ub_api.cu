@@ -41,6 +41,10 @@ struct ub_sim {
   cudaStream_t aux[ub::kMaxSplit - 1]; cudaEvent_t ev_fork, ev_join[ub::kMaxSplit - 1];   // extra streams: the parts of a round overlap their tails
   uint32_t nsplit, ndsplit;     // parts of the main group / of the drift group (together <= kMaxSplit)
   uint32_t round_no;            // launches alternate between two ticket counters
+  // ub_run replays a captured CUDA graph of kGraphRounds rounds while the configuration of a round (parts, lists,
+  // iterations per launch) stays the same: small jobs are bound by launch latency
+  cudaGraphExec_t graph; uint64_t graph_key; uint32_t graph_launches;
+  cudaStream_t gstream; cudaEvent_t ev_g;   // the graph's origin stream when the caller's is the default stream (which cannot be captured)
   float last_ms; uint32_t last_launches;
 };
 
@@ -48,6 +52,8 @@ struct ub_sim {
 
 static int compact_live(ub_sim* s, uint64_t* live, bool any_state);
 static int set_dev(const ub_sim* s) { return cudaSetDevice(s->cfg.device) == cudaSuccess ? UB_OK : UB_ECUDA; }
+// (a captured graph holds kernel arguments by value: device pointers, list lengths)
+static void drop_graph(ub_sim* s) { if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; } s->graph_key = 0; }
 
 const char* ub_strerror(int e) {
   switch (e) {
@@ -94,6 +100,7 @@ int ub_create(const ub_config* c, ub_sim** out) {
   s->d_TR = nullptr; s->d_lut = nullptr;
   s->last_ms = 0.f; s->last_launches = 0;
   s->use_list = false; s->ndrift = 0; s->drift_livecnt = 0;
+  s->graph = nullptr; s->graph_key = 0; s->graph_launches = 0;
   // parts of a round (each on a stream of its own; together with the drift group's at most kMaxSplit).  Measured: config 5
   // (65536 replicas) 2 parts 5.9e10, 4 parts 5.5e10 request-steps/s; config 3 (4096 replicas, whole job) 1 part 1.18e10,
   // 2 parts 1.31e10, 4 parts 1.22e10 at one iteration per launch and 2.61e10 / 3.29e10 / 3.34e10 at 64; config 2 (3072
@@ -120,7 +127,8 @@ int ub_create(const ub_config* c, ub_sim** out) {
     ub_destroy(s);
     return UB_ECUDA;
   }
-  bool aux_ok = true;
+  bool aux_ok = cudaStreamCreateWithFlags(&s->gstream, cudaStreamNonBlocking) == cudaSuccess &&
+                cudaEventCreateWithFlags(&s->ev_g, cudaEventDisableTiming) == cudaSuccess;
   for (uint32_t i = 0; i + 1 < kMaxSplit; i++)
     aux_ok = aux_ok && cudaStreamCreateWithFlags(&s->aux[i], cudaStreamNonBlocking) == cudaSuccess &&
              cudaEventCreateWithFlags(&s->ev_join[i], cudaEventDisableTiming) == cudaSuccess;
@@ -153,6 +161,9 @@ void ub_destroy(ub_sim* s) {
   cudaFree(s->d_neu); cudaFree(s->d_hist); cudaFree(s->d_stats); cudaFree(s->d_word);
   cudaFree(s->d_list); cudaFree(s->d_count); cudaFree(s->d_evbuf); cudaFree(s->d_live); cudaFree(s->d_livecnt); cudaFree(s->d_drift); cudaFree(s->d_drift_live);
   cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);
+  if (s->graph) cudaGraphExecDestroy(s->graph);
+  if (s->gstream) cudaStreamDestroy(s->gstream);
+  if (s->ev_g) cudaEventDestroy(s->ev_g);
   if (s->h_word) cudaFreeHost(s->h_word);
   if (s->ev0) cudaEventDestroy(s->ev0);
   if (s->ev1) cudaEventDestroy(s->ev1);
@@ -262,6 +273,7 @@ int ub_set_replicas(ub_sim* s, const ub_replica* reps) {
   }
   s->have_reps = false;
   s->use_list = false;                             // (a rewound run: every replica is live again)
+  drop_graph(s);
   cudaFree(s->d_ada_ring); cudaFree(s->d_ada_state); cudaFree(s->d_ada_grid);        // adaptation is set per replica table
   s->d_ada_ring = nullptr; s->d_ada_state = nullptr; s->d_ada_grid = nullptr; s->h_ada_grid.clear();
   s->dev.ada_ring = nullptr; s->dev.ada_state = nullptr; s->dev.ada_grid = nullptr;
@@ -424,6 +436,62 @@ static int issue_steps(ub_sim* s, uint64_t n_iters, uint32_t* launches, const in
   return cudaGetLastError() == cudaSuccess ? UB_OK : UB_ECUDA;
 }
 
+// ub_run's rounds through a CUDA graph: kGraphRounds rounds (their launches on all the part streams, the fork / join
+// events and the hand-over flush behind them) are captured once from issue_steps() itself and replayed; the graph is
+// kept while the round configuration -- list mode, list lengths, iterations per launch -- is unchanged.  An even
+// number of rounds, so the alternation of the two ticket counters is the same in every replay.
+constexpr uint32_t kGraphRounds = 64;
+static int issue_steps_graphed(ub_sim* s, uint64_t n_iters, uint32_t* launches) {
+  const uint32_t ipl = s->cfg.iters_per_launch > 1 ? s->cfg.iters_per_launch : 1;
+  const uint64_t per = (uint64_t)kGraphRounds * ipl;
+  if (s->d_ada_ring || n_iters < per || n_iters % per || (s->round_no & 1u)) return issue_steps(s, n_iters, launches);
+  uint64_t key = 0x9E3779B97F4A7C15ull ^ ipl;
+  auto mix = [&](uint64_t v) { key = (key ^ v) * 0xBF58476D1CE4E5B9ull; key ^= key >> 29; };
+  mix(s->use_list ? 1u : 0u); mix(s->ndrift); mix(s->drift_livecnt);
+  for (uint32_t i = 0; i < s->nsplit; i++) mix(s->use_list ? s->livecnt[i] : 0u);
+  key |= 1ull;
+  // the default streams cannot be captured: the graph then starts from a stream of the library's, ordered behind the
+  // caller's stream and in front of it again by events
+  cudaStream_t user = s->stream;
+  const bool own = user == nullptr || user == cudaStreamLegacy || user == cudaStreamPerThread;
+  struct Swap { ub_sim* s; cudaStream_t user; ~Swap() { s->stream = user; } } swap{s, user};
+  if (own) {
+    CK(cudaEventRecord(s->ev_g, user));
+    CK(cudaStreamWaitEvent(s->gstream, s->ev_g, 0));
+    s->stream = s->gstream;
+  }
+  if (!s->graph || s->graph_key != key) {
+    if (s->graph) { cudaGraphExecDestroy(s->graph); s->graph = nullptr; }
+    cudaGraph_t g = nullptr;
+    const uint32_t round0 = s->round_no;
+    if (cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+      cudaGetLastError(); s->stream = user;
+      return issue_steps(s, n_iters, launches);
+    }
+    uint32_t nl = 0;
+    const int rc = issue_steps(s, per, &nl);
+    const cudaError_t e = cudaStreamEndCapture(s->stream, &g);
+    s->round_no = round0;
+    if (rc != UB_OK || e != cudaSuccess || !g || cudaGraphInstantiate(&s->graph, g, 0) != cudaSuccess) {
+      cudaGetLastError();
+      if (g) cudaGraphDestroy(g);
+      s->graph = nullptr; s->stream = user;
+      return issue_steps(s, n_iters, launches);
+    }
+    cudaGraphDestroy(g);
+    s->graph_key = key; s->graph_launches = nl;
+  }
+  const uint64_t reps = n_iters / per;
+  for (uint64_t i = 0; i < reps; i++) CK(cudaGraphLaunch(s->graph, s->stream));
+  s->round_no += (uint32_t)(reps * kGraphRounds);
+  *launches = (uint32_t)(reps * s->graph_launches);
+  if (own) {
+    CK(cudaEventRecord(s->ev_g, s->gstream));
+    CK(cudaStreamWaitEvent(user, s->ev_g, 0));
+  }
+  return UB_OK;
+}
+
 static int read_live(ub_sim* s, uint64_t* live) {
   launch_count_live(s->d_count, s->cfg.n_replicas, s->d_word, s->stream);
   CK(cudaMemcpyAsync(s->h_word, s->d_word, 8, cudaMemcpyDeviceToHost, s->stream));
@@ -492,7 +560,7 @@ int ub_run(ub_sim* s, uint64_t max_iters, uint64_t* iters_done) {
     const uint64_t k = (max_iters - done) < chunk ? (max_iters - done) : chunk;
     uint32_t nl = 0;
     CK(cudaEventRecord(s->ev0, s->stream));
-    rc = issue_steps(s, k, &nl);
+    rc = done ? issue_steps_graphed(s, k, &nl) : issue_steps(s, k, &nl);     // (the first rounds also set the kernels up)
     CK(cudaEventRecord(s->ev1, s->stream));
     if (rc) return rc;
     done += k; total_launches += nl;
@@ -608,6 +676,7 @@ int ub_set_gamma_ada(ub_sim* s, const ub_gamma_ada* g, const uint8_t* adaptive) 
   }
   // commit
   cudaFree(s->d_lut);
+  drop_graph(s);
   s->d_lut = n_lut; s->d_ada_ring = n_ring; s->d_ada_state = n_state; s->d_ada_grid = n_grid;
   s->h_lut.swap(lut); s->h_lut_off.swap(lut_off); s->h_lut_nb.swap(lut_nb);
   SimDev& d = s->dev;

@@ -389,6 +389,36 @@ def test_specialised_and_generic_instances_agree(gpu, oracle_mod, ipl):
     spec.close(); gen.close(); o.close()
 
 
+@pytest.mark.parametrize("own_stream", [False, True], ids=["default-stream", "own-stream"])
+def test_run_replays_a_graph_and_survives_a_rewind(gpu, oracle_mod, own_stream):
+    """ub_run replays a captured CUDA graph of 64 rounds (from a stream of the library's when the caller's is the default
+    stream).  The graph holds device pointers by value: ub_set_replicas (which re-allocates the boost tables) must drop
+    it.  Same digests as the oracle before and after the rewind, and after changing the replica table."""
+    import torch
+    wl = W.config2(n_seeds=40)
+    tr = wl.traces(workers=4)
+    st = torch.cuda.Stream() if own_stream else torch.cuda.current_stream()
+    g = gpu.Sim(wl.sim, wl.replicas, tr, stream=st.cuda_stream)
+    o = oracle_mod.OracleSim(wl.sim, wl.replicas, tr)
+    o.run()
+    issued = g.run()
+    assert issued >= 1024                                           # (several graph replays)
+    want = o.digest()
+    assert np.array_equal(g.digest(), want)
+    gpu._chk(gpu.lib().ub_set_replicas(g._h, gpu.make_replicas(wl.replicas, wl.R)))      # rewind
+    g.run()
+    assert np.array_equal(g.digest(), want)
+    rep2 = {k: v.copy() for k, v in wl.replicas.items()}
+    rep2["gamma"][:] = 2.0                                          # other boost tables, same shapes
+    gpu._chk(gpu.lib().ub_set_replicas(g._h, gpu.make_replicas(rep2, wl.R)))
+    g.run()
+    o2 = oracle_mod.OracleSim(wl.sim, rep2, tr)
+    o2.run()
+    assert np.array_equal(g.digest(), o2.digest())
+    assert not np.array_equal(o2.digest(), want)
+    g.close(); o.close(); o2.close()
+
+
 # ------------------------------------------------------------------------------------------ streaming kernel, randomised
 
 @pytest.mark.parametrize("seed", range(8))
