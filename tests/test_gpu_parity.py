@@ -449,6 +449,34 @@ def test_stream_path_randomised(gpu, oracle_mod, seed):
     assert max(s["peak_active"] for s in o.stats()) > 64
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_drift_path_randomised(gpu, oracle_mod, seed):
+    """The drift instance's territory (SRPT, LAS: keys move with every token; SJF, SPF beside them), with and without
+    MemGuard: windows of several hundred requests, so that its decode-run and waiting-tail phases (order checks against
+    the keys written so far), the general path and evictions all occur; 1 or 3 iterations per launch."""
+    rng = np.random.default_rng([78, seed])
+    n, NT = 700, 3
+    P = rng.integers(1, 400, (NT, n)); D = rng.integers(1, 160, (NT, n))
+    gaps = rng.exponential(2500, (NT, n)) * rng.choice([0.05, 1.0, 3.0], (NT, n), p=[0.3, 0.5, 0.2])
+    a = np.cumsum(gaps, axis=1).astype(np.int64)
+    R = 12
+    rep = W.make_replicas(R, trace_id=np.arange(R) % NT,
+                          policy=rng.choice([W.POLICY_SRPT, W.POLICY_LAS, W.POLICY_SJF, W.POLICY_SPF], R, p=[0.4, 0.4, 0.1, 0.1]),
+                          guard=rng.integers(0, 2, R), hysteresis_us=0)
+    blk = 16
+    kvb = int(rng.integers(60, 400))
+    D = np.minimum(D, np.maximum(1, kvb * blk - P))
+    sim = dict(kv_blocks=kvb, queue_cap=int(rng.choice([400, 700])), max_batch=int(rng.choice([8, 48, 256])),
+               chunk_tokens=int(rng.choice([16, 64, 512])), token_budget=int(rng.choice([64, 256, 1024])),
+               bin_tokens=int(rng.choice([16, 64, 256])), preempt_mode=int(rng.integers(0, 3)),
+               swap_pool_blocks=int(rng.integers(0, 200)))
+    wl = W.custom(a, P, D, sim, rep)
+    g, o = _pair(gpu, oracle_mod, wl, ipl=int(rng.choice([1, 3])))
+    g.run(); o.run()
+    _assert_same(g, o, f"randomised drift case {seed}: {sim}")
+    assert max(s["peak_active"] for s in o.stats()) > 64
+
+
 # ------------------------------------------------------------------------------------------ kernel-level parity: a1 score
 
 @pytest.mark.parametrize("policy", [W.POLICY_FCFS, W.POLICY_SRPT, W.POLICY_BOOST, W.POLICY_LAS, W.POLICY_SJF,
