@@ -961,9 +961,11 @@ template <bool ADA, bool MULTI, bool LIST, bool DRIFT, bool SPEC> static void la
   const uint32_t need = (A.rend - A.rbeg + kSWarps - 1) / kSWarps;
   uint32_t grid = (uint32_t)(sms * ctas_per_sm);
   if (grid > need) grid = need;
-  // a warp takes 7/8 of an even share of the replicas by static striding, the rest by tickets (measured on config 5:
-  // 1/2 7.4e10, 3/4 8.15e10, 7/8 8.32e10, 15/16 8.29e10, all static 7.97e10 request-steps/s)
-  const uint32_t nwarps = grid * kSWarps, share = ((A.rend - A.rbeg) / nwarps) * 7u / 8u;
+  // a warp takes 15/16 of an even share of the replicas by static striding (7/8 with several iterations per launch), the
+  // rest by tickets (measured on config 5, the generic instance: 1/2 7.4e10, 3/4 8.15e10, 7/8 8.32e10, 15/16 8.29e10, all
+  // static 7.97e10 request-steps/s; the BOOST + MemGuard instance: 13/16 8.27e10, 7/8 8.54e10, 15/16 .. 61/64 8.60e10,
+  // the resident mode 1.03e11 at 7/8 and 1.005e11 at 15/16)
+  const uint32_t nwarps = grid * kSWarps, share = ((A.rend - A.rbeg) / nwarps) * (MULTI ? 14u : 15u) / 16u;
   A.nstat = share > 2u ? share : 2u;
   A.dynbase = A.rbeg + A.nstat * nwarps;
   k_stream<ADA, MULTI, LIST, DRIFT, SPEC><<<grid, 32 * kSWarps, 0, st>>>(A);
