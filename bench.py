@@ -271,7 +271,7 @@ def whole_job(B, wl, traces, stream, peak, label):
 def gamma_ada_probe(B, w4, tr4, stream, iters=4096):
     """Config 4 (distribution shift + memory pressure, 16384 replicas) for `iters` iterations from its loaded phase, once
     as the static gamma sweep and once with gamma-Ada on every replica: what a round costs when UPDATEGAMMA (k_gamma_ada,
-    one CTA per replica) and the hand-over of re-keyed replicas to the team kernels (k_step) run every round."""
+    one warp per replica) and the hand-over of re-keyed replicas to the team kernels (k_step) run every round."""
     out = {}
     R = int(w4.sim["n_replicas"])
     for label, ada in (("static", None), ("gamma_ada", dict(window=256, min_samples=32, beta_shift=3, levels=32,
